@@ -1,0 +1,143 @@
+/* tdde.h -- C ABI of the B200 Crank-Nicolson / BiCGSTAB Dirac propagator (libtdde.so).
+ *
+ * One thing is computed: the implicit Crank-Nicolson step of the time-dependent Dirac equation in a
+ * (kappa,mu) x radial-B-spline basis (Eq. 25, with H at the midpoint of PAPER.md:195, Eq. 22)
+ *
+ *     (S + i dt/2 H(t_{n+1/2})) c^{n+1} = (S - i dt/2 H(t_{n+1/2})) c^n ,
+ *     H(t) = H0 + sum_L g_L(t) (A_L (x) R_L)                     (block form: Eq. 17)
+ *
+ * solved by BiCGSTAB preconditioned with M = S + i dt/2 H0 (Eq. 26),
+ * which is block-diagonal over angular channels and is applied through per-class
+ * banded LU factors.  The assembled matrix H(t) is never stored.
+ *
+ * Conventions (all entry points):
+ *   - "host" / "device" is stated per pointer.  Device pointers are plain CUDA device addresses
+ *     (e.g. torch.Tensor.data_ptr()), 16-byte aligned; the library neither frees nor keeps them.
+ *   - state vectors: c[a * n_rad + j], a = angular channel (one (kappa,mu) pair), j = radial index over
+ *     both components, complex128 interleaved (re, im), contiguous, length n = n_ang * n_rad.
+ *   - a radial band matrix R of half-bandwidth w: row-major band[i][d + w] = R[i][i + d], -w <= d <= w,
+ *     entries with i + d outside [0, n_rad) are ignored.
+ *   - every call returns 0 on success or a negative tdde_status; nothing throws or aborts across the ABI.
+ *   - all device work is enqueued on the CUDA stream given to tdde_create.
+ *   - there is no CPU fallback: every call fails with TDDE_ECUDA when no CUDA device is usable.
+ */
+#ifndef TDDE_H_
+#define TDDE_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tdde_handle tdde_handle;        /* opaque; owned by the library, freed by tdde_destroy */
+typedef struct { double re, im; } tdde_c64;    /* == numpy complex128 */
+
+typedef enum {
+  TDDE_OK         =  0,
+  TDDE_EINVAL     = -1,  /* null pointer, non-positive dims, w >= n_rad, CSR column out of range, bad rowptr, bad class */
+  TDDE_ENOMEM     = -2,  /* host or device allocation failed */
+  TDDE_ECUDA      = -3,  /* a CUDA runtime call failed; text via tdde_last_cuda_error() */
+  TDDE_ESINGULAR  = -4,  /* zero / non-finite pivot in the banded LU of some M_k = S_k + i dt/2 H0_k */
+  TDDE_EBREAKDOWN = -5,  /* |rho|, |<rhat,v>| or <t,t> below 1e-290 or non-finite (BiCGSTAB breakdown) */
+  TDDE_ENOCONV    = -6   /* max_iter full iterations without reaching rtol */
+} tdde_status;
+
+typedef struct {
+  int32_t n_ang;     /* angular channels (kappa,mu)                                  PAPER.md:94 (Eq. 7)   */
+  int32_t n_rad;     /* 2*N_r: radial index over both components, interleaved                               */
+  int32_t n_cls;     /* distinct field-free blocks (kappa-classes), 1..n_ang          */
+  int32_t w0;        /* half-bandwidth of S_k and H0_k                                                      */
+  int32_t n_terms;   /* T, number of coupling terms g_L (A_L (x) R_L); may be 0                             */
+  int32_t max_iter;  /* full BiCGSTAB iterations per step before TDDE_ENOCONV                               */
+  double  dt;        /* time step (a.u.); may be negative (time reversal)                                   */
+  double  rtol;      /* stop when ||r||_2 <= rtol * ||b||_2                                                 */
+} tdde_config;
+
+typedef struct {               /* one coupling term g_L(t) * (A_L (x) R_L)      PAPER.md:155-163 (Eq. 17)   */
+  int32_t w;                   /* half-bandwidth of R_L                                                     */
+  int32_t reserved;            /* set to 0                                                                  */
+  const tdde_c64* R_band;      /* host [n_rad][2w+1]                                                        */
+  const int32_t*  A_rowptr;    /* host CSR of A_L, n_ang + 1 entries, non-decreasing, A_rowptr[0] = 0       */
+  const int32_t*  A_col;       /* host [nnz], 0 <= col < n_ang                                              */
+  const tdde_c64* A_val;       /* host [nnz]                                                                */
+} tdde_term;
+
+typedef struct {
+  int64_t steps;        /* CN steps completed by the call                                                   */
+  int64_t half_iters;   /* BiCGSTAB half-iterations summed over those steps (a full iteration counts 2;
+                           the ||s|| exit leaves an odd count for its step)                                 */
+  int64_t applies;      /* operator applies (A or B times a vector) enqueued and executed                   */
+  int64_t preconds;     /* preconditioner applies executed                                                  */
+  double  rel_res;      /* ||r|| / ||b|| at the exit of the last step                                       */
+  int32_t status;       /* tdde_status of the last step                                                     */
+  int32_t last_half_iters; /* half-iterations of the last step                                              */
+} tdde_stats;
+
+/* Build a propagator.  Copies every host input (caller may free them on return), forms per class
+ * M+-_k = S_k +- i dt/2 H0_k, factorises M+_k = L U without pivoting (legitimate because the Hermitian part
+ * of M+_k is S_k > 0), allocates ~10 work vectors of n complex128 on the current device.
+ *   S_band, H0_band : host [n_cls][n_rad][2*w0+1]
+ *   cls_of_chan     : host [n_ang], values in [0, n_cls)
+ *   terms           : host [n_terms]
+ *   cuda_stream     : cudaStream_t (as void*), 0 = legacy default stream
+ * Errors: TDDE_EINVAL, TDDE_ENOMEM, TDDE_ECUDA, TDDE_ESINGULAR; *out is NULL on failure. */
+int tdde_create(tdde_handle** out, const tdde_config* cfg, const tdde_c64* S_band, const tdde_c64* H0_band,
+                const int32_t* cls_of_chan, const tdde_term* terms, void* cuda_stream);
+
+/* One CN step in place on c_dev (device, n complex128).  g_mid: host [n_terms], g_L(t_{n+1/2}).
+ * If st != NULL the call synchronises the stream and fills *st; otherwise solver failures are latched and
+ * returned by the next synchronising call.  On failure c_dev holds the last iterate. */
+int tdde_step(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, tdde_stats* st);
+
+/* n_steps CN steps in place on c_dev.  g_table: host [n_steps][n_terms], row s = g_L at the midpoint of step s.
+ * Stops at the first failing step (st->steps tells how many completed).  Synchronises iff st != NULL. */
+int tdde_propagate(tdde_handle* h, tdde_c64* c_dev, int64_t n_steps, const double* g_table, tdde_stats* st);
+
+/* *out (host) = Re(c^H S c), the total probability in the non-orthogonal basis (S: PAPER.md:178-182).
+ * Synchronises. */
+int tdde_norm(tdde_handle* h, const tdde_c64* c_dev, double* out);
+
+/* Test / measurement export: y = alpha S x + beta (H0 + sum_L g[L] A_L (x) R_L) x.
+ * g: host [n_terms] (may be NULL when n_terms == 0).  x_dev, y_dev: device, n complex128, must not alias.
+ * Does not synchronise. */
+int tdde_apply(tdde_handle* h, tdde_c64 alpha, tdde_c64 beta, const double* g, const tdde_c64* x_dev,
+               tdde_c64* y_dev);
+
+/* Test / measurement export: y = (S + i dt/2 H0)^{-1} x, block-Jacobi over channels.
+ * x_dev, y_dev: device, n complex128; may alias.  Does not synchronise. */
+int tdde_precond(tdde_handle* h, const tdde_c64* x_dev, tdde_c64* y_dev);
+
+/* Same as tdde_step / tdde_propagate but with HOST state vectors: c_host (n complex128) is copied to the
+ * device, propagated and copied back; synchronises.  This is the end-to-end entry bench.py's "e2e" times. */
+int tdde_propagate_host(tdde_handle* h, tdde_c64* c_host, int64_t n_steps, const double* g_table, tdde_stats* st);
+
+/* Pin P11 support: one CN step that runs exactly n_iters full BiCGSTAB iterations with every exit test
+ * disabled.  trace_dev (device, nullable): [n_iters][8][n] complex128 receiving, after each iteration, the
+ * vectors p, v, s, t, x, r, y, z (this order, boundary layout).  Synchronises. */
+int tdde_step_forced(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, int32_t n_iters, tdde_c64* trace_dev);
+
+/* Measurement helpers (timed in bench.py; no effect on state).
+ *   tdde_time_kernel: enqueue `reps` launches of one internal kernel on the handle's stream between two CUDA
+ *   events and return the mean milliseconds per launch in *ms_out.  which: 0 = operator apply v = A y with
+ *   fused <rhat,v>; 1 = preconditioner apply; 2 = p-update; 3 = s-update; 4 = x,r-update; 5 = boundary<->internal
+ *   transpose; 6 = S-only apply (norm).  g: host [n_terms] used by which == 0.  Synchronises.
+ *   tdde_fp64_peak: run an unrolled independent-DFMA kernel on every SM and return achieved FLOP/s. */
+int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, const double* g, double* ms_out);
+int tdde_fp64_peak(void* cuda_stream, double* flops_out);
+
+/* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
+int64_t tdde_launch_count(const tdde_handle* h);
+
+/* Which operator-apply kernel the handle uses: 1 = banded-A register-resident fast path, 0 = generic CSR path. */
+int tdde_apply_path(const tdde_handle* h);
+
+void        tdde_destroy(tdde_handle* h);          /* NULL is allowed */
+const char* tdde_strerror(int status);             /* static string */
+const char* tdde_last_cuda_error(void);            /* text of the last CUDA failure seen by this thread */
+int         tdde_version(void);                    /* ABI version, currently 1 */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TDDE_H_ */

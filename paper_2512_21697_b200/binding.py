@@ -1,0 +1,246 @@
+"""Thin ctypes binding over libtdde.so (include/tdde.h).  Argument marshalling only: every step of the hot path
+runs in the library's CUDA kernels.  torch is used for device memory and streams, nothing else.
+
+The names mirror the C ABI: ``Tdde.step / propagate / norm / apply / precond`` call ``tdde_step`` etc.
+There is no CPU fallback: importing works without a GPU (so that the ABI can be inspected), but creating a
+propagator without a CUDA device raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtdde.so")
+
+EXPORTS = [
+    "tdde_create", "tdde_step", "tdde_propagate", "tdde_norm", "tdde_apply", "tdde_precond",
+    "tdde_propagate_host", "tdde_step_forced", "tdde_time_kernel", "tdde_fp64_peak", "tdde_launch_count",
+    "tdde_apply_path", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
+]
+
+STATUS = {0: "TDDE_OK", -1: "TDDE_EINVAL", -2: "TDDE_ENOMEM", -3: "TDDE_ECUDA", -4: "TDDE_ESINGULAR",
+          -5: "TDDE_EBREAKDOWN", -6: "TDDE_ENOCONV"}
+
+
+class tdde_c64(C.Structure):
+    _fields_ = [("re", C.c_double), ("im", C.c_double)]
+
+
+class tdde_config(C.Structure):
+    _fields_ = [("n_ang", C.c_int32), ("n_rad", C.c_int32), ("n_cls", C.c_int32), ("w0", C.c_int32),
+                ("n_terms", C.c_int32), ("max_iter", C.c_int32), ("dt", C.c_double), ("rtol", C.c_double)]
+
+
+class tdde_term(C.Structure):
+    _fields_ = [("w", C.c_int32), ("reserved", C.c_int32), ("R_band", C.c_void_p), ("A_rowptr", C.c_void_p),
+                ("A_col", C.c_void_p), ("A_val", C.c_void_p)]
+
+
+class tdde_stats(C.Structure):
+    _fields_ = [("steps", C.c_int64), ("half_iters", C.c_int64), ("applies", C.c_int64), ("preconds", C.c_int64),
+                ("rel_res", C.c_double), ("status", C.c_int32), ("last_half_iters", C.c_int32)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class TddeError(RuntimeError):
+    def __init__(self, status: int, where: str, detail: str = ""):
+        self.status = status
+        super().__init__(f"{where}: {STATUS.get(status, status)} ({detail})" if detail else f"{where}: {STATUS.get(status, status)}")
+
+
+_lib = None
+
+
+def load_library(path: Optional[str] = None) -> C.CDLL:
+    """dlopen libtdde.so and declare the prototypes.  Raises if the library has not been built."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = path or LIB_PATH
+    if not os.path.exists(p):
+        raise RuntimeError(f"{p} is missing: build it with `python -m paper_2512_21697_b200.build` "
+                           "(there is no CPU fallback)")
+    lib = C.CDLL(p)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    lib.tdde_create.argtypes = [C.POINTER(vp), C.POINTER(tdde_config), vp, vp, vp, C.POINTER(tdde_term), vp]
+    lib.tdde_step.argtypes = [vp, vp, vp, C.POINTER(tdde_stats)]
+    lib.tdde_propagate.argtypes = [vp, vp, i64, vp, C.POINTER(tdde_stats)]
+    lib.tdde_propagate_host.argtypes = [vp, vp, i64, vp, C.POINTER(tdde_stats)]
+    lib.tdde_norm.argtypes = [vp, vp, C.POINTER(dbl)]
+    lib.tdde_apply.argtypes = [vp, tdde_c64, tdde_c64, vp, vp, vp]
+    lib.tdde_precond.argtypes = [vp, vp, vp]
+    lib.tdde_step_forced.argtypes = [vp, vp, vp, i32, vp]
+    lib.tdde_time_kernel.argtypes = [vp, i32, i32, vp, C.POINTER(dbl)]
+    lib.tdde_fp64_peak.argtypes = [vp, C.POINTER(dbl)]
+    lib.tdde_launch_count.argtypes = [vp]
+    lib.tdde_launch_count.restype = i64
+    lib.tdde_apply_path.argtypes = [vp]
+    lib.tdde_destroy.argtypes = [vp]
+    lib.tdde_destroy.restype = None
+    lib.tdde_strerror.argtypes = [C.c_int]
+    lib.tdde_strerror.restype = C.c_char_p
+    lib.tdde_last_cuda_error.restype = C.c_char_p
+    for name in ("tdde_create", "tdde_step", "tdde_propagate", "tdde_propagate_host", "tdde_norm", "tdde_apply",
+                 "tdde_precond", "tdde_step_forced", "tdde_time_kernel", "tdde_fp64_peak", "tdde_apply_path",
+                 "tdde_version"):
+        getattr(lib, name).restype = C.c_int
+    if path is None:
+        _lib = lib
+    return lib
+
+
+def _check(lib, rc: int, where: str):
+    if rc != 0:
+        detail = lib.tdde_last_cuda_error().decode() if rc == -3 else lib.tdde_strerror(rc).decode()
+        raise TddeError(rc, where, detail)
+
+
+def _np_ptr(a: np.ndarray) -> int:
+    return a.ctypes.data
+
+
+def _g_array(g, n_terms: int, rows: Optional[int] = None) -> np.ndarray:
+    g = np.ascontiguousarray(np.asarray(g, dtype=np.float64))
+    want = n_terms if rows is None else rows * n_terms
+    if g.size != want:
+        raise ValueError(f"g has {g.size} entries, expected {want}")
+    return g
+
+
+class Tdde:
+    """One propagator handle (tdde_create ... tdde_destroy) for a tdde_inputs.Problem-like object."""
+
+    def __init__(self, problem, dt: Optional[float] = None, rtol: Optional[float] = None,
+                 max_iter: Optional[int] = None, stream=None, device: str = "cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the TDDE propagator has no CPU fallback")
+        self.lib = load_library()
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.n_ang, self.n_rad, self.n_terms = problem.n_ang, problem.n_rad, problem.n_terms
+        self.n = problem.n_ang * problem.n_rad
+        cfg = tdde_config(problem.n_ang, problem.n_rad, problem.n_cls, problem.w0, problem.n_terms,
+                          int(problem.max_iter if max_iter is None else max_iter),
+                          float(problem.dt if dt is None else dt), float(problem.rtol if rtol is None else rtol))
+        S = np.ascontiguousarray(problem.S_band, dtype=np.complex128)
+        H0 = np.ascontiguousarray(problem.H0_band, dtype=np.complex128)
+        cls = np.ascontiguousarray(problem.cls_of_chan, dtype=np.int32)
+        keep = [S, H0, cls]
+        terms = (tdde_term * max(1, problem.n_terms))()
+        for L, t in enumerate(problem.terms):
+            R = np.ascontiguousarray(t.R_band, dtype=np.complex128)
+            rp = np.ascontiguousarray(t.A_rowptr, dtype=np.int32)
+            col = np.ascontiguousarray(t.A_col, dtype=np.int32)
+            val = np.ascontiguousarray(t.A_val, dtype=np.complex128)
+            keep += [R, rp, col, val]
+            terms[L] = tdde_term(int(t.w), 0, _np_ptr(R), _np_ptr(rp), _np_ptr(col), _np_ptr(val))
+        h = C.c_void_p()
+        rc = self.lib.tdde_create(C.byref(h), C.byref(cfg), _np_ptr(S), _np_ptr(H0), _np_ptr(cls), terms,
+                                  C.c_void_p(self.stream.cuda_stream))
+        _check(self.lib, rc, "tdde_create")
+        self.h = h
+
+    # -- helpers --
+    def to_device(self, c: np.ndarray):
+        t = self.torch.from_numpy(np.ascontiguousarray(c, dtype=np.complex128))
+        return t.to(self.device)
+
+    def _vec(self, t, name="vector"):
+        if t.dtype != self.torch.complex128 or not t.is_cuda or not t.is_contiguous() or t.numel() != self.n:
+            raise ValueError(f"{name} must be a contiguous CUDA complex128 tensor of {self.n} elements")
+        return C.c_void_p(t.data_ptr())
+
+    # -- C ABI mirrors --
+    def step(self, c_dev, g_mid, want_stats: bool = True):
+        g = _g_array(g_mid, self.n_terms)
+        st = tdde_stats()
+        rc = self.lib.tdde_step(self.h, self._vec(c_dev), _np_ptr(g), C.byref(st) if want_stats else None)
+        _check(self.lib, rc, "tdde_step")
+        return st.as_dict()
+
+    def propagate(self, c_dev, g_table, n_steps: Optional[int] = None, check: bool = True):
+        g = np.asarray(g_table, dtype=np.float64)
+        n_steps = (g.shape[0] if g.ndim == 2 else 1) if n_steps is None else n_steps
+        g = _g_array(g, self.n_terms, n_steps)
+        st = tdde_stats()
+        rc = self.lib.tdde_propagate(self.h, self._vec(c_dev), n_steps, _np_ptr(g), C.byref(st))
+        if check:
+            _check(self.lib, rc, "tdde_propagate")
+        out = st.as_dict()
+        out["rc"] = rc
+        return out
+
+    def propagate_host(self, c_host: np.ndarray, g_table, n_steps: int):
+        if c_host.dtype != np.complex128 or not c_host.flags.c_contiguous or c_host.size != self.n:
+            raise ValueError("c_host must be a contiguous complex128 array of n elements")
+        g = _g_array(g_table, self.n_terms, n_steps)
+        st = tdde_stats()
+        rc = self.lib.tdde_propagate_host(self.h, _np_ptr(c_host), n_steps, _np_ptr(g), C.byref(st))
+        _check(self.lib, rc, "tdde_propagate_host")
+        return st.as_dict()
+
+    def norm(self, c_dev) -> float:
+        out = C.c_double()
+        _check(self.lib, self.lib.tdde_norm(self.h, self._vec(c_dev), C.byref(out)), "tdde_norm")
+        return out.value
+
+    def apply(self, alpha: complex, beta: complex, g, x_dev, y_dev=None):
+        g = _g_array(g, self.n_terms) if self.n_terms else np.zeros(1)
+        y = self.torch.empty_like(x_dev) if y_dev is None else y_dev
+        a, b = complex(alpha), complex(beta)
+        rc = self.lib.tdde_apply(self.h, tdde_c64(a.real, a.imag), tdde_c64(b.real, b.imag), _np_ptr(g),
+                                 self._vec(x_dev, "x"), self._vec(y, "y"))
+        _check(self.lib, rc, "tdde_apply")
+        return y
+
+    def precond(self, x_dev, y_dev=None):
+        y = self.torch.empty_like(x_dev) if y_dev is None else y_dev
+        _check(self.lib, self.lib.tdde_precond(self.h, self._vec(x_dev, "x"), self._vec(y, "y")), "tdde_precond")
+        return y
+
+    def step_forced(self, c_dev, g_mid, n_iters: int, trace: bool = True):
+        g = _g_array(g_mid, self.n_terms)
+        tr = self.torch.empty((n_iters, 8, self.n), dtype=self.torch.complex128, device=self.device) if trace else None
+        rc = self.lib.tdde_step_forced(self.h, self._vec(c_dev), _np_ptr(g), n_iters,
+                                       C.c_void_p(tr.data_ptr()) if trace else None)
+        _check(self.lib, rc, "tdde_step_forced")
+        return tr
+
+    def time_kernel(self, which: int, reps: int, g=None) -> float:
+        garr = _g_array(g, self.n_terms) if (g is not None and self.n_terms) else np.zeros(max(1, self.n_terms))
+        out = C.c_double()
+        _check(self.lib, self.lib.tdde_time_kernel(self.h, which, reps, _np_ptr(garr), C.byref(out)), "tdde_time_kernel")
+        return out.value
+
+    def fp64_peak(self) -> float:
+        out = C.c_double()
+        _check(self.lib, self.lib.tdde_fp64_peak(C.c_void_p(self.stream.cuda_stream), C.byref(out)), "tdde_fp64_peak")
+        return out.value
+
+    @property
+    def launch_count(self) -> int:
+        return int(self.lib.tdde_launch_count(self.h))
+
+    @property
+    def apply_path(self) -> str:
+        return "banded" if self.lib.tdde_apply_path(self.h) == 1 else "generic"
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.tdde_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,308 @@
+// tdde_create.cu -- tdde_create / tdde_destroy: validation, band repacking, per-class banded LU (host, one-time),
+// device allocation.  SURVEY 8(a) a0; PAPER.md:211-215 (Eq. 26), :268, :275-276 ("performed at start-up").
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include "tdde_handle.h"
+
+thread_local std::string g_last_cuda_error;
+
+int tdde_cuda_fail(cudaError_t e, const char* what) {
+  g_last_cuda_error = std::string(cudaGetErrorName(e)) + ": " + cudaGetErrorString(e) + " in " + what;
+  cudaGetLastError();
+  return e == cudaErrorMemoryAllocation ? TDDE_ENOMEM : TDDE_ECUDA;
+}
+
+namespace {
+
+template <class T>
+int dev_upload(T** dst, const T* src, size_t count, cudaStream_t s) {
+  *dst = nullptr;
+  if (count == 0) count = 1, src = nullptr;
+  CU(cudaMalloc((void**)dst, count * sizeof(T)));
+  if (src) CU(cudaMemcpyAsync(*dst, src, count * sizeof(T), cudaMemcpyHostToDevice, s));
+  else CU(cudaMemsetAsync(*dst, 0, count * sizeof(T), s));
+  return 0;
+}
+
+// row-band [n][2w+1] (band[i][d+w] = M[i][i+d]) -> column-band col[j][e] = M[j-w+e][j], zero outside the matrix
+void row_to_col_band(const zc* row, zc* col, int n, int w) {
+  const int nd = 2 * w + 1;
+  for (int j = 0; j < n; ++j)
+    for (int e = 0; e < nd; ++e) {
+      const int i = j - w + e;
+      col[(size_t)j * nd + e] = (i >= 0 && i < n) ? row[(size_t)i * nd + (2 * w - e)] : zc(0, 0);
+    }
+}
+
+// LU without pivoting of one band matrix given as row-band; fills Lcol [n][w], Ucol [n][w+1] (tdde_internal.h).
+// No fill leaves the band.  Returns false on a zero / non-finite pivot.
+bool band_lu(std::vector<zc>& M, int n, int w, zc* Lcol, zc* Ucol) {
+  const int nd = 2 * w + 1;
+  auto at = [&](int i, int j) -> zc& { return M[(size_t)i * nd + (j - i + w)]; };
+  for (int i = 0; i < n; ++i) {
+    const zc piv = at(i, i);
+    if (!(std::isfinite(piv.real()) && std::isfinite(piv.imag())) || std::abs(piv) < TDDE_TINY) return false;
+    const int last = std::min(i + w, n - 1);
+    for (int r = i + 1; r <= last; ++r) {
+      const zc l = at(r, i) / piv;
+      at(r, i) = l;
+      for (int c = i + 1; c <= last; ++c) at(r, c) -= l * at(i, c);
+    }
+  }
+  for (int i = 0; i < n; ++i) {
+    for (int d = 1; d <= w; ++d) Lcol[(size_t)i * w + d - 1] = (i + d < n) ? at(i + d, i) : zc(0, 0);
+    Ucol[(size_t)i * (w + 1)] = zc(1, 0) / at(i, i);
+    for (int d = 1; d <= w; ++d) Ucol[(size_t)i * (w + 1) + d] = (i - d >= 0) ? at(i - d, i) : zc(0, 0);
+  }
+  return true;
+}
+
+int validate(const tdde_config* c, const tdde_c64* S, const tdde_c64* H0, const int32_t* cls, const tdde_term* terms) {
+  if (!c || !S || !H0 || !cls) return TDDE_EINVAL;
+  if (c->n_ang <= 0 || c->n_rad <= 0 || c->n_cls <= 0 || c->n_cls > c->n_ang) return TDDE_EINVAL;
+  if (c->w0 < 1 || c->w0 > 32 || c->w0 >= c->n_rad) return TDDE_EINVAL;
+  if (c->n_terms < 0 || c->n_terms > TDDE_MAX_TERMS || (c->n_terms > 0 && !terms)) return TDDE_EINVAL;
+  if (c->max_iter <= 0 || !(c->rtol >= 0) || !std::isfinite(c->dt) || c->dt == 0.0) return TDDE_EINVAL;
+  if ((long long)c->n_ang * c->n_rad > (1LL << 40)) return TDDE_EINVAL;
+  for (int a = 0; a < c->n_ang; ++a)
+    if (cls[a] < 0 || cls[a] >= c->n_cls) return TDDE_EINVAL;
+  for (int L = 0; L < c->n_terms; ++L) {
+    const tdde_term& t = terms[L];
+    if (t.w < 0 || t.w > 32 || t.w >= c->n_rad || !t.R_band || !t.A_rowptr) return TDDE_EINVAL;
+    if (t.A_rowptr[0] != 0) return TDDE_EINVAL;
+    for (int a = 0; a < c->n_ang; ++a)
+      if (t.A_rowptr[a + 1] < t.A_rowptr[a]) return TDDE_EINVAL;
+    const int nnz = t.A_rowptr[c->n_ang];
+    if (nnz > 0 && (!t.A_col || !t.A_val)) return TDDE_EINVAL;
+    for (int q = 0; q < nnz; ++q)
+      if (t.A_col[q] < 0 || t.A_col[q] >= c->n_ang) return TDDE_EINVAL;
+  }
+  return 0;
+}
+
+// Is every A_L banded with offsets 1..m_L, m_L = m0 + ms * L, and is a kernel instantiated for that shape?
+bool detect_banded(const tdde_config* c, const tdde_term* terms, int* m0, int* ms) {
+  const int T = c->n_terms;
+  if (!apply_banded_available(0, 0, 0, c->w0)) return false;   // the S-only apply needs the T = 0 kernel too
+  if (T == 0) { *m0 = *ms = 0; return true; }
+  int m[TDDE_MAX_TERMS];
+  for (int L = 0; L < T; ++L) {
+    if (terms[L].w != c->w0) return false;
+    m[L] = 0;
+    for (int a = 0; a < c->n_ang; ++a)
+      for (int q = terms[L].A_rowptr[a]; q < terms[L].A_rowptr[a + 1]; ++q) {
+        const int o = terms[L].A_col[q] - a;
+        if (o == 0) return false;
+        m[L] = std::max(m[L], std::abs(o));
+      }
+    if (m[L] == 0) return false;
+  }
+  // duplicates in a CSR row would need summing: reject (generic path sums them naturally)
+  for (int L = 0; L < T; ++L)
+    for (int a = 0; a < c->n_ang; ++a)
+      for (int q = terms[L].A_rowptr[a] + 1; q < terms[L].A_rowptr[a + 1]; ++q)
+        for (int q2 = terms[L].A_rowptr[a]; q2 < q; ++q2)
+          if (terms[L].A_col[q] == terms[L].A_col[q2]) return false;
+  const int cand_ms[2] = {T > 1 ? m[1] - m[0] : 1, 0};
+  for (int t = 0; t < (T > 1 ? 1 : 2); ++t) {
+    bool ok = true;
+    for (int L = 0; L < T; ++L) ok = ok && (m[L] == m[0] + cand_ms[t] * L);
+    if (ok && apply_banded_available(T, m[0], cand_ms[t], c->w0)) { *m0 = m[0]; *ms = cand_ms[t]; return true; }
+  }
+  return false;
+}
+
+}  // namespace
+
+extern "C" void tdde_destroy(tdde_handle* h) {
+  if (!h) return;
+  cudaStreamSynchronize(h->stream);
+  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Lcol, h->d_Ucol, h->X, h->r,
+                  h->rhat, h->p, h->v, h->s, h->t, h->y, h->z, h->c_stage, h->d_st, h->d_st_bench, h->d_partials,
+                  h->d_ticket, h->d_g, h->d_g_small, h->d_zero_g};
+  for (void* p : ptrs) if (p) cudaFree(p);
+  for (int L = 0; L < TDDE_MAX_TERMS; ++L) {
+    if (h->d_R[L]) cudaFree(h->d_R[L]);
+    if (h->d_Arowptr[L]) cudaFree(h->d_Arowptr[L]);
+    if (h->d_Acol[L]) cudaFree(h->d_Acol[L]);
+    if (h->d_Aval[L]) cudaFree(h->d_Aval[L]);
+  }
+  if (h->h_st) cudaFreeHost(h->h_st);
+  cudaGetLastError();
+  delete h;
+}
+
+static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H0_band, const int32_t* cls_of_chan,
+                       const tdde_term* terms) {
+  const tdde_config& c = h->cfg;
+  cudaStream_t s = h->stream;
+  const int n_rad = c.n_rad, w0 = c.w0, nd0 = 2 * w0 + 1, T = c.n_terms;
+  h->ld = (c.n_ang + 31) / 32 * 32;
+  h->nint = (long long)n_rad * h->ld;
+  h->n = (long long)c.n_ang * n_rad;
+  h->tau = 0.5 * c.dt;
+  h->blk_count = (long long)c.n_cls * n_rad * nd0;
+
+  int m0 = 0, ms = 0;
+  h->path = detect_banded(&c, terms, &m0, &ms) ? 1 : 0;
+  h->bT = T; h->bM0 = m0; h->bMS = ms; h->bW = w0;
+  h->norm_banded = (h->path == 1);
+
+  // radial segment length: enough thread blocks to fill 148 SMs several times, yet long enough that the
+  // 2W halo rows recomputed per segment stay a small fraction
+  {
+    const int chan_blocks = (h->ld + 127) / 128;
+    int want_segs = (148 * 4 + chan_blocks - 1) / chan_blocks;
+    int seg = (n_rad + want_segs - 1) / want_segs;
+    seg = std::max(seg, 4 * w0);
+    h->seg_len = std::min(seg, n_rad);
+  }
+
+  const zc* S = reinterpret_cast<const zc*>(S_band);
+  const zc* H0 = reinterpret_cast<const zc*>(H0_band);
+  const size_t blk_sz = (size_t)n_rad * nd0;
+
+  // classes per channel (pads -> class 0)
+  {
+    std::vector<int> cls(h->ld, 0);
+    for (int a = 0; a < c.n_ang; ++a) cls[a] = cls_of_chan[a];
+    int rc = dev_upload(&h->d_cls, cls.data(), cls.size(), s);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(s));
+  }
+  // block bands S, H0, M+ in the layout of the chosen path; LU of M+
+  {
+    std::vector<zc> Sx(h->blk_count), Hx(h->blk_count), Mx(h->blk_count);
+    std::vector<zc> Lc((size_t)c.n_cls * n_rad * w0), Uc((size_t)c.n_cls * n_rad * (w0 + 1));
+    std::vector<zc> Mrow(blk_sz);
+    const zc itau(0.0, h->tau);
+    for (int k = 0; k < c.n_cls; ++k) {
+      const zc* Sk = S + k * blk_sz;
+      const zc* Hk = H0 + k * blk_sz;
+      for (size_t q = 0; q < blk_sz; ++q) Mrow[q] = Sk[q] + itau * Hk[q];
+      // entries that point outside the matrix are ignored by contract: zero them so they cannot enter the LU
+      for (int i = 0; i < n_rad; ++i)
+        for (int d = -w0; d <= w0; ++d)
+          if (i + d < 0 || i + d >= n_rad) Mrow[(size_t)i * nd0 + d + w0] = zc(0, 0);
+      if (h->path == 1) {
+        row_to_col_band(Sk, &Sx[k * blk_sz], n_rad, w0);
+        row_to_col_band(Hk, &Hx[k * blk_sz], n_rad, w0);
+        row_to_col_band(Mrow.data(), &Mx[k * blk_sz], n_rad, w0);
+      } else {
+        std::memcpy(&Sx[k * blk_sz], Sk, blk_sz * sizeof(zc));
+        std::memcpy(&Hx[k * blk_sz], Hk, blk_sz * sizeof(zc));
+        std::memcpy(&Mx[k * blk_sz], Mrow.data(), blk_sz * sizeof(zc));
+      }
+      if (!band_lu(Mrow, n_rad, w0, &Lc[(size_t)k * n_rad * w0], &Uc[(size_t)k * n_rad * (w0 + 1)]))
+        return TDDE_ESINGULAR;
+    }
+    int rc;
+    if ((rc = dev_upload(&h->d_S, reinterpret_cast<cplx*>(Sx.data()), Sx.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_H0, reinterpret_cast<cplx*>(Hx.data()), Hx.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_Mp, reinterpret_cast<cplx*>(Mx.data()), Mx.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_blk_tmp, (cplx*)nullptr, Mx.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_Lcol, reinterpret_cast<cplx*>(Lc.data()), Lc.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_Ucol, reinterpret_cast<cplx*>(Uc.data()), Uc.size(), s))) return rc;
+    CU(cudaStreamSynchronize(s));
+  }
+  // coupling terms
+  if (h->path == 1 && T > 0) {
+    int nslots = 0;
+    for (int L = 0; L < T; ++L) nslots += 2 * (m0 + ms * L);
+    std::vector<zc> Aoff((size_t)nslots * h->ld, zc(0, 0));
+    int slot0 = 0;
+    for (int L = 0; L < T; ++L) {
+      const int m = m0 + ms * L;
+      const zc* val = reinterpret_cast<const zc*>(terms[L].A_val);
+      for (int a = 0; a < c.n_ang; ++a)
+        for (int q = terms[L].A_rowptr[a]; q < terms[L].A_rowptr[a + 1]; ++q) {
+          const int o = terms[L].A_col[q] - a;
+          const int qq = o < 0 ? o + m : m + o - 1;
+          Aoff[(size_t)(slot0 + qq) * h->ld + a] = val[q];
+        }
+      slot0 += 2 * m;
+    }
+    int rc = dev_upload(&h->d_Aoff, reinterpret_cast<cplx*>(Aoff.data()), Aoff.size(), s);
+    if (rc) return rc;
+    CU(cudaStreamSynchronize(s));
+  }
+  for (int L = 0; L < T; ++L) {
+    const int w = terms[L].w, nd = 2 * w + 1;
+    h->w[L] = w;
+    const zc* R = reinterpret_cast<const zc*>(terms[L].R_band);
+    std::vector<zc> Rx((size_t)n_rad * nd);
+    if (h->path == 1) row_to_col_band(R, Rx.data(), n_rad, w);
+    else std::memcpy(Rx.data(), R, Rx.size() * sizeof(zc));
+    int rc;
+    if ((rc = dev_upload(&h->d_R[L], reinterpret_cast<cplx*>(Rx.data()), Rx.size(), s))) return rc;
+    if (h->path == 0) {
+      const int nnz = terms[L].A_rowptr[c.n_ang];
+      std::vector<int> rp(h->ld + 1, nnz);
+      for (int a = 0; a <= c.n_ang; ++a) rp[a] = terms[L].A_rowptr[a];
+      if ((rc = dev_upload(&h->d_Arowptr[L], rp.data(), rp.size(), s))) return rc;
+      if ((rc = dev_upload(&h->d_Acol[L], terms[L].A_col, (size_t)nnz, s))) return rc;
+      if ((rc = dev_upload(&h->d_Aval[L], reinterpret_cast<const cplx*>(terms[L].A_val), (size_t)nnz, s))) return rc;
+    }
+    CU(cudaStreamSynchronize(s));
+  }
+  // work vectors
+  cplx** vecs[] = {&h->X, &h->r, &h->rhat, &h->p, &h->v, &h->s, &h->t, &h->y, &h->z};
+  for (cplx** v : vecs) {
+    CU(cudaMalloc((void**)v, (size_t)h->nint * sizeof(cplx)));
+    CU(cudaMemsetAsync(*v, 0, (size_t)h->nint * sizeof(cplx), s));
+  }
+  // state and scratch
+  CU(cudaMalloc((void**)&h->d_st, sizeof(SolverState)));
+  CU(cudaMalloc((void**)&h->d_st_bench, sizeof(SolverState)));
+  CU(cudaMallocHost((void**)&h->h_st, sizeof(SolverState)));
+  std::memset(h->h_st, 0, sizeof(SolverState));
+  h->h_st->rtol2 = c.rtol * c.rtol;
+  h->h_st->max_half = 2 * c.max_iter;
+  h->h_st->done = 1;
+  CU(cudaMemcpyAsync(h->d_st, h->h_st, sizeof(SolverState), cudaMemcpyHostToDevice, s));
+  CU(cudaStreamSynchronize(s));
+  {
+    SolverState b;
+    std::memset(&b, 0, sizeof(b));
+    b.rho = b.rho_old = b.alpha = b.omega = b.beta = make_double2(1.0, 0.0);
+    b.force = 1; b.max_half = 1 << 30; b.nb2 = 1.0;
+    CU(cudaMemcpy(h->d_st_bench, &b, sizeof(b), cudaMemcpyHostToDevice));
+  }
+  CU(cudaMalloc((void**)&h->d_partials, (size_t)TDDE_MAX_PARTIAL_BLOCKS * 4 * sizeof(double)));
+  CU(cudaMalloc((void**)&h->d_ticket, sizeof(unsigned int)));
+  CU(cudaMemsetAsync(h->d_ticket, 0, sizeof(unsigned int), s));
+  const size_t tcount = T > 0 ? T : 1;
+  CU(cudaMalloc((void**)&h->d_g_small, tcount * sizeof(double)));
+  CU(cudaMalloc((void**)&h->d_zero_g, tcount * sizeof(double)));
+  CU(cudaMemsetAsync(h->d_zero_g, 0, tcount * sizeof(double), s));
+  CU(cudaMemsetAsync(h->d_g_small, 0, tcount * sizeof(double), s));
+  CU(cudaStreamSynchronize(s));
+  return 0;
+}
+
+extern "C" int tdde_create(tdde_handle** out, const tdde_config* cfg, const tdde_c64* S_band, const tdde_c64* H0_band,
+                           const int32_t* cls_of_chan, const tdde_term* terms, void* cuda_stream) {
+  if (!out) return TDDE_EINVAL;
+  *out = nullptr;
+  int rc = validate(cfg, S_band, H0_band, cls_of_chan, terms);
+  if (rc) return rc;
+  int ndev = 0;
+  CU(cudaGetDeviceCount(&ndev));
+  if (ndev <= 0) { g_last_cuda_error = "no CUDA device"; return TDDE_ECUDA; }
+  tdde_handle* h = new (std::nothrow) tdde_handle();
+  if (!h) return TDDE_ENOMEM;
+  h->cfg = *cfg;
+  h->stream = (cudaStream_t)cuda_stream;
+  try {
+    rc = create_impl(h, S_band, H0_band, cls_of_chan, terms);
+  } catch (const std::bad_alloc&) {
+    rc = TDDE_ENOMEM;
+  } catch (...) {
+    rc = TDDE_EINVAL;
+  }
+  if (rc) { tdde_destroy(h); return rc; }
+  *out = h;
+  return 0;
+}

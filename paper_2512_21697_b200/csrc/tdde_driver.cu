@@ -1,0 +1,264 @@
+// tdde_driver.cu -- the Crank-Nicolson / BiCGSTAB step driver and the remaining C-ABI entry points.
+//
+// Control flow without a host sync per iteration (SURVEY 7 hard part 3): every step enqueues its two
+// start-of-step applies, `nspec` speculated BiCGSTAB iterations and a one-thread "close" kernel.  Kernels of
+// an iteration are no-ops once the device-side `done` flag is set; if the speculated iterations were not
+// enough, close latches `stalled`, every later kernel (including later steps) becomes a no-op, and the host
+// finds out at its next state read (once per batch of steps), resumes that step with more iterations and
+// raises nspec.  All BiCGSTAB scalars stay in SolverState on the device.
+#include <algorithm>
+#include <cstring>
+#include "tdde_handle.h"
+
+static const cplx* blk_ptr(const tdde_handle* h, int blk) {
+  switch (blk) {
+    case BLK_S: return h->d_S;
+    case BLK_H0: return h->d_H0;
+    case BLK_MP: return h->d_Mp;
+    default: return h->d_blk_tmp;
+  }
+}
+
+int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int blk, cplx beta, bool with_terms,
+                  const double* g_dev, const int* step_ptr, int guard, int fin, SolverState* st) {
+  ApplyArgs a;
+  std::memset(&a, 0, sizeof(a));
+  a.x = x; a.y = y; a.aux = aux;
+  a.n_ang = h->cfg.n_ang; a.n_rad = h->cfg.n_rad; a.ld = h->ld;
+  a.seg_len = h->seg_len;
+  a.cls = h->d_cls;
+  a.beta = beta;
+  a.g = g_dev; a.step_ptr = step_ptr;
+  a.w0 = h->cfg.w0;
+  a.guard = guard;
+  a.red.partials = h->d_partials; a.red.ticket = h->d_ticket; a.red.st = st; a.red.fin = fin;
+  const int T = with_terms ? h->cfg.n_terms : 0;
+  a.n_terms = T;
+  int rc;
+  const bool banded = (h->path == 1);
+  if (banded) {
+    a.blk = blk_ptr(h, blk);
+    for (int L = 0; L < T; ++L) a.Rcol[L] = h->d_R[L];
+    a.Aoff = h->d_Aoff;
+    rc = launch_apply_banded(a, T, h->bM0, h->bMS, h->cfg.w0, h->stream);
+  } else {
+    a.blk_row = blk_ptr(h, blk);
+    for (int L = 0; L < T; ++L) {
+      a.Rrow[L] = h->d_R[L]; a.w[L] = h->w[L];
+      a.A_rowptr[L] = h->d_Arowptr[L]; a.A_col[L] = h->d_Acol[L]; a.A_val[L] = h->d_Aval[L];
+    }
+    rc = launch_apply_generic(a, h->stream);
+  }
+  if (rc < 0) return TDDE_EINVAL;
+  h->launches += rc;
+  return 0;
+}
+
+int enqueue_precond(tdde_handle* h, const cplx* x, cplx* y, const SolverState* st) {
+  PrecArgs p;
+  p.x = x; p.y = y; p.n_ang = h->cfg.n_ang; p.n_rad = h->cfg.n_rad; p.ld = h->ld; p.w = h->cfg.w0;
+  p.cls = h->d_cls; p.Lcol = h->d_Lcol; p.Ucol = h->d_Ucol; p.st = st;
+  int rc = launch_precond(p, h->stream);
+  if (rc < 0) return TDDE_EINVAL;
+  h->launches += rc;
+  return 0;
+}
+
+VecArgs make_vec_args(tdde_handle* h, SolverState* st, int fin) {
+  VecArgs a;
+  a.n = h->nint;
+  a.x = h->X; a.r = h->r; a.rhat = h->rhat; a.p = h->p; a.v = h->v; a.s = h->s; a.t = h->t; a.y = h->y; a.z = h->z;
+  a.b = h->s;   // start of step: S c lands in the s buffer, H c in the t buffer (both free until the iteration)
+  a.u = h->t;
+  a.dt = h->cfg.dt;
+  a.red.partials = h->d_partials; a.red.ticket = h->d_ticket; a.red.st = st; a.red.fin = fin;
+  return a;
+}
+
+int sync_state(tdde_handle* h) {
+  CU(cudaMemcpyAsync(h->h_st, h->d_st, sizeof(SolverState), cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return 0;
+}
+
+// The two start-of-step applies and the initial residual (SURVEY 8(a) a2 + a3): with x0 = c,
+//   b = S c - i tau H c,   r0 = b - (S c + i tau H c) = -i dt H c,
+// so one H-apply (t buffer) and one S-apply (s buffer) give both; b itself is only needed through ||b||.
+static int enqueue_step_start(tdde_handle* h) {
+  SolverState* st = h->d_st;
+  const cplx one = make_double2(1.0, 0.0);
+  int rc;
+  if ((rc = enqueue_apply(h, h->X, h->t, nullptr, BLK_H0, one, true, h->d_g, &st->step_idx, 2, FIN_NONE, st))) return rc;
+  if ((rc = enqueue_apply(h, h->X, h->s, nullptr, BLK_S, one, false, h->d_zero_g, nullptr, 2, FIN_NONE, st))) return rc;
+  h->launches += launch_vec_r0(make_vec_args(h, st, FIN_R0), h->stream);
+  return 0;
+}
+
+// One full BiCGSTAB iteration in the order of SURVEY 8(c) C4.
+static int enqueue_iteration(tdde_handle* h) {
+  SolverState* st = h->d_st;
+  const cplx itau = make_double2(0.0, h->tau);
+  int rc;
+  h->launches += launch_vec_p(make_vec_args(h, st, FIN_NONE), h->stream);                 // p = r + beta (p - omega v)
+  if ((rc = enqueue_precond(h, h->p, h->y, st))) return rc;                               // y = M^-1 p
+  if ((rc = enqueue_apply(h, h->y, h->v, h->rhat, BLK_MP, itau, true, h->d_g, &st->step_idx, 1, FIN_ALPHA, st))) return rc;
+  h->launches += launch_vec_s(make_vec_args(h, st, FIN_S), h->stream);                    // s = r - alpha v, ||s||
+  h->launches += launch_vec_halfexit(make_vec_args(h, st, FIN_NONE), h->stream);          // x += alpha y on the ||s|| exit
+  if ((rc = enqueue_precond(h, h->s, h->z, st))) return rc;                               // z = M^-1 s
+  if ((rc = enqueue_apply(h, h->z, h->t, h->s, BLK_MP, itau, true, h->d_g, &st->step_idx, 1, FIN_OMEGA, st))) return rc;
+  h->launches += launch_vec_xr(make_vec_args(h, st, FIN_R), h->stream);                   // x, r updates, ||r||, <rhat,r>
+  return 0;
+}
+
+static int upload_g(tdde_handle* h, const double* g_table, long long n_steps) {
+  const int T = h->cfg.n_terms;
+  if (T == 0) { if (!h->d_g) { CU(cudaMalloc((void**)&h->d_g, sizeof(double))); h->g_cap = 1; } return 0; }
+  if (n_steps > h->g_cap) {
+    if (h->d_g) { CU(cudaStreamSynchronize(h->stream)); cudaFree(h->d_g); h->d_g = nullptr; }
+    CU(cudaMalloc((void**)&h->d_g, (size_t)n_steps * T * sizeof(double)));
+    h->g_cap = n_steps;
+  }
+  CU(cudaMemcpyAsync(h->d_g, g_table, (size_t)n_steps * T * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+  return 0;
+}
+
+static void fill_stats(const tdde_handle* h, tdde_stats* st) {
+  if (!st) return;
+  const SolverState* s = h->h_st;
+  st->steps = s->steps_done; st->half_iters = s->total_half; st->applies = s->applies; st->preconds = s->preconds;
+  st->rel_res = s->last_rel_res; st->status = s->status; st->last_half_iters = s->last_half_iters;
+}
+
+// X (internal layout) holds c; advance n_steps steps.  Always ends with one state read.
+static int run_steps(tdde_handle* h, long long n_steps) {
+  const long long batch = 64;
+  long long enq = 0;          // steps enqueued so far (== steps_done when nothing stalled)
+  int rc;
+  h->launches += launch_step_open(h->d_st, 0, 0, 0, h->stream);
+  while (true) {
+    const long long upto = std::min(n_steps, enq + batch);
+    for (; enq < upto; ++enq) {
+      if ((rc = enqueue_step_start(h))) return rc;
+      for (int it = 0; it < h->nspec; ++it)
+        if ((rc = enqueue_iteration(h))) return rc;
+      h->launches += launch_step_close(h->d_st, h->stream);
+    }
+    if ((rc = sync_state(h))) return rc;
+    CU(cudaGetLastError());
+    if (h->h_st->status != 0) return h->h_st->status;
+    while (h->h_st->stalled) {
+      // the step after steps_done ran out of speculated iterations: resume it
+      h->launches += launch_step_open(h->d_st, 0, 0, 1, h->stream);
+      const int more = std::max(2, h->nspec);
+      for (int it = 0; it < more; ++it)
+        if ((rc = enqueue_iteration(h))) return rc;
+      h->launches += launch_step_close(h->d_st, h->stream);
+      if ((rc = sync_state(h))) return rc;
+      if (h->h_st->status != 0) return h->h_st->status;
+      if (!h->h_st->stalled) {
+        const int need = (h->h_st->last_half_iters + 1) / 2;
+        h->nspec = std::min(h->cfg.max_iter, std::max(h->nspec, need));
+      }
+      enq = h->h_st->steps_done;      // steps after the stalled one were no-ops: redo them
+    }
+    if (h->h_st->steps_done >= n_steps) return 0;
+    enq = h->h_st->steps_done;
+  }
+}
+
+extern "C" int tdde_propagate(tdde_handle* h, tdde_c64* c_dev, int64_t n_steps, const double* g_table, tdde_stats* st) {
+  if (!h || !c_dev || n_steps < 0 || (n_steps > 0 && h->cfg.n_terms > 0 && !g_table)) return TDDE_EINVAL;
+  if (st) std::memset(st, 0, sizeof(*st));
+  if (n_steps == 0) return 0;
+  int rc;
+  if ((rc = upload_g(h, g_table, n_steps))) return rc;
+  // a failure latched by an earlier call is cleared here: each call reports its own status
+  h->h_st->status = 0; h->h_st->stalled = 0; h->h_st->done = 1; h->h_st->force = 0;
+  h->h_st->rtol2 = h->cfg.rtol * h->cfg.rtol; h->h_st->max_half = 2 * h->cfg.max_iter;
+  CU(cudaMemcpyAsync(h->d_st, h->h_st, sizeof(SolverState), cudaMemcpyHostToDevice, h->stream));
+  h->launches += launch_to_internal(reinterpret_cast<const cplx*>(c_dev), h->X, h->cfg.n_ang, h->cfg.n_rad, h->ld, h->stream);
+  rc = run_steps(h, n_steps);
+  h->launches += launch_to_boundary(h->X, reinterpret_cast<cplx*>(c_dev), h->cfg.n_ang, h->cfg.n_rad, h->ld, h->stream);
+  CU(cudaStreamSynchronize(h->stream));
+  fill_stats(h, st);
+  return rc;
+}
+
+extern "C" int tdde_step(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, tdde_stats* st) {
+  return tdde_propagate(h, c_dev, 1, g_mid, st);
+}
+
+extern "C" int tdde_propagate_host(tdde_handle* h, tdde_c64* c_host, int64_t n_steps, const double* g_table, tdde_stats* st) {
+  if (!h || !c_host) return TDDE_EINVAL;
+  const size_t bytes = (size_t)h->n * sizeof(cplx);
+  if (!h->c_stage) CU(cudaMalloc((void**)&h->c_stage, bytes));
+  CU(cudaMemcpyAsync(h->c_stage, c_host, bytes, cudaMemcpyHostToDevice, h->stream));
+  int rc = tdde_propagate(h, reinterpret_cast<tdde_c64*>(h->c_stage), n_steps, g_table, st);
+  CU(cudaMemcpyAsync(c_host, h->c_stage, bytes, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return rc;
+}
+
+extern "C" int tdde_step_forced(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, int32_t n_iters, tdde_c64* trace_dev) {
+  if (!h || !c_dev || n_iters < 0 || (h->cfg.n_terms > 0 && !g_mid)) return TDDE_EINVAL;
+  int rc;
+  if ((rc = upload_g(h, g_mid, 1))) return rc;
+  h->h_st->status = 0; h->h_st->stalled = 0; h->h_st->done = 1;
+  CU(cudaMemcpyAsync(h->d_st, h->h_st, sizeof(SolverState), cudaMemcpyHostToDevice, h->stream));
+  const int na = h->cfg.n_ang, nr = h->cfg.n_rad;
+  h->launches += launch_to_internal(reinterpret_cast<const cplx*>(c_dev), h->X, na, nr, h->ld, h->stream);
+  h->launches += launch_step_open(h->d_st, 0, 1, 0, h->stream);
+  if ((rc = enqueue_step_start(h))) return rc;
+  for (int it = 0; it < n_iters; ++it) {
+    if ((rc = enqueue_iteration(h))) return rc;
+    if (trace_dev) {
+      const cplx* vecs[8] = {h->p, h->v, h->s, h->t, h->X, h->r, h->y, h->z};
+      for (int q = 0; q < 8; ++q) {
+        cplx* dst = reinterpret_cast<cplx*>(trace_dev) + ((size_t)it * 8 + q) * (size_t)h->n;
+        h->launches += launch_to_boundary(vecs[q], dst, na, nr, h->ld, h->stream);
+      }
+    }
+  }
+  h->launches += launch_to_boundary(h->X, reinterpret_cast<cplx*>(c_dev), na, nr, h->ld, h->stream);
+  if ((rc = sync_state(h))) return rc;
+  const int status = h->h_st->status;
+  // leave the state idle and unforced for the next call
+  h->h_st->status = 0; h->h_st->force = 0; h->h_st->done = 1;
+  CU(cudaMemcpyAsync(h->d_st, h->h_st, sizeof(SolverState), cudaMemcpyHostToDevice, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  return status;
+}
+
+extern "C" int tdde_norm(tdde_handle* h, const tdde_c64* c_dev, double* out) {
+  if (!h || !c_dev || !out) return TDDE_EINVAL;
+  int rc;
+  h->launches += launch_to_internal(reinterpret_cast<const cplx*>(c_dev), h->y, h->cfg.n_ang, h->cfg.n_rad, h->ld, h->stream);
+  if ((rc = enqueue_apply(h, h->y, h->z, h->y, BLK_S, make_double2(0, 0), false, h->d_zero_g, nullptr, 0, FIN_NORM, h->d_st))) return rc;
+  if ((rc = sync_state(h))) return rc;
+  *out = h->h_st->norm_out;
+  return 0;
+}
+
+extern "C" int tdde_apply(tdde_handle* h, tdde_c64 alpha, tdde_c64 beta, const double* g, const tdde_c64* x_dev, tdde_c64* y_dev) {
+  if (!h || !x_dev || !y_dev || x_dev == y_dev || (h->cfg.n_terms > 0 && !g)) return TDDE_EINVAL;
+  int rc;
+  if (h->cfg.n_terms > 0)
+    CU(cudaMemcpyAsync(h->d_g_small, g, h->cfg.n_terms * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+  h->launches += launch_combine_blocks(h->d_S, h->d_H0, make_double2(alpha.re, alpha.im),
+                                       make_double2(beta.re, beta.im), h->d_blk_tmp, h->blk_count, h->stream);
+  h->launches += launch_to_internal(reinterpret_cast<const cplx*>(x_dev), h->y, h->cfg.n_ang, h->cfg.n_rad, h->ld, h->stream);
+  if ((rc = enqueue_apply(h, h->y, h->z, nullptr, BLK_TMP, make_double2(beta.re, beta.im), true, h->d_g_small, nullptr, 0, FIN_NONE, h->d_st))) return rc;
+  h->launches += launch_to_boundary(h->z, reinterpret_cast<cplx*>(y_dev), h->cfg.n_ang, h->cfg.n_rad, h->ld, h->stream);
+  CU(cudaGetLastError());
+  return 0;
+}
+
+extern "C" int tdde_precond(tdde_handle* h, const tdde_c64* x_dev, tdde_c64* y_dev) {
+  if (!h || !x_dev || !y_dev) return TDDE_EINVAL;
+  int rc;
+  h->launches += launch_to_internal(reinterpret_cast<const cplx*>(x_dev), h->y, h->cfg.n_ang, h->cfg.n_rad, h->ld, h->stream);
+  if ((rc = enqueue_precond(h, h->y, h->z, nullptr))) return rc;
+  h->launches += launch_to_boundary(h->z, reinterpret_cast<cplx*>(y_dev), h->cfg.n_ang, h->cfg.n_rad, h->ld, h->stream);
+  CU(cudaGetLastError());
+  return 0;
+}

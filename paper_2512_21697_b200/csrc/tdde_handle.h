@@ -1,0 +1,70 @@
+// tdde_handle.h -- the opaque handle behind tdde.h and the host-side helpers shared by the API files.
+#pragma once
+#include <complex>
+#include <string>
+#include <vector>
+#include "tdde_internal.h"
+
+typedef std::complex<double> zc;
+
+struct tdde_handle {
+  tdde_config cfg;
+  cudaStream_t stream = nullptr;
+  int ld = 0;                    // padded channel count (multiple of 32)
+  long long nint = 0;            // n_rad * ld
+  long long n = 0;               // n_ang * n_rad
+  double tau = 0;                // dt / 2
+
+  // apply path
+  int path = 0;                  // 1 banded fast path, 0 generic
+  int bT = 0, bM0 = 0, bMS = 0, bW = 0;
+  int seg_len = 0;               // radial rows per thread (banded path)
+  bool norm_banded = false;      // S-only apply can use the banded T=0 kernel
+
+  // device constants
+  int* d_cls = nullptr;                      // [ld]
+  cplx *d_S = nullptr, *d_H0 = nullptr, *d_Mp = nullptr, *d_blk_tmp = nullptr;   // block bands in the path's layout
+  long long blk_count = 0;                   // n_cls * n_rad * (2 w0 + 1)
+  cplx* d_R[TDDE_MAX_TERMS] = {};            // per term band in the path's layout (col-band or row-band)
+  int w[TDDE_MAX_TERMS] = {};
+  cplx* d_Aoff = nullptr;                    // banded path
+  int* d_Arowptr[TDDE_MAX_TERMS] = {};       // generic path
+  int* d_Acol[TDDE_MAX_TERMS] = {};
+  cplx* d_Aval[TDDE_MAX_TERMS] = {};
+  cplx *d_Lcol = nullptr, *d_Ucol = nullptr; // preconditioner factors
+
+  // work vectors (internal layout)
+  cplx *X = nullptr, *r = nullptr, *rhat = nullptr, *p = nullptr, *v = nullptr, *s = nullptr, *t = nullptr,
+       *y = nullptr, *z = nullptr;
+  cplx* c_stage = nullptr;                   // boundary-layout device buffer for tdde_propagate_host
+
+  // solver state, scratch
+  SolverState* d_st = nullptr;
+  SolverState* d_st_bench = nullptr;         // never-idle dummy state for tdde_time_kernel
+  SolverState* h_st = nullptr;               // pinned mirror
+  double* d_partials = nullptr;
+  unsigned int* d_ticket = nullptr;
+  double* d_g = nullptr;                     // [g_cap][T]
+  long long g_cap = 0;
+  double* d_g_small = nullptr;               // [T] for tdde_apply
+  double* d_zero_g = nullptr;                // [T] zeros
+  int nspec = 2;                             // speculated iterations per step
+  long long launches = 0;
+};
+
+extern thread_local std::string g_last_cuda_error;
+int tdde_cuda_fail(cudaError_t e, const char* what);
+
+#define CU(call)                                               \
+  do {                                                         \
+    cudaError_t e__ = (call);                                  \
+    if (e__ != cudaSuccess) return tdde_cuda_fail(e__, #call); \
+  } while (0)
+
+// enqueue helpers (tdde_driver.cu)
+enum BlkSel { BLK_S = 0, BLK_H0 = 1, BLK_MP = 2, BLK_TMP = 3 };
+int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int blk, cplx beta, bool with_terms,
+                  const double* g_dev, const int* step_ptr, int guard, int fin, SolverState* st);
+int enqueue_precond(tdde_handle* h, const cplx* x, cplx* y, const SolverState* st);
+VecArgs make_vec_args(tdde_handle* h, SolverState* st, int fin);
+int sync_state(tdde_handle* h);

@@ -1,0 +1,121 @@
+// tdde_internal.h -- private declarations shared by the host API and the kernel translation units.
+//
+// Internal layout ("channel-fastest"): element (radial j, channel a) of a vector lives at X[j * ld + a],
+// ld = n_ang rounded up to a multiple of 32.  Lanes of a warp then own consecutive channels: radial band
+// coefficients R_L[i][j] are warp-uniform, the angular coefficients A_L[a'][a'+o] are per-lane registers
+// and the vector accesses are coalesced 16-byte loads.  Pad channels (a >= n_ang) hold zeros throughout.
+// The boundary layout (tdde.h) is channel-major; transposes happen at entry/exit of the API calls.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "tdde.h"
+
+#define TDDE_MAX_TERMS 8
+#define TDDE_MAX_PARTIAL_BLOCKS 65536
+#define TDDE_TINY 1e-290
+
+typedef double2 cplx;
+
+// ---- device-resident solver state: every BiCGSTAB scalar and flag lives here ----
+struct SolverState {
+  cplx rho, rho_old, alpha, omega, beta;   // C4 notation
+  double nb2;          // ||b||^2
+  double res2;         // ||r||^2 or ||s||^2 of the latest test
+  double rtol2;        // rtol^2
+  double norm_out;     // tdde_norm result
+  int done;            // this step's solve finished (converged or failed)
+  int status;          // latched tdde_status (0 = ok)
+  int stalled;         // speculated iterations ran out before convergence; later kernels are no-ops
+  int half_exit;       // 1: ||s|| exit taken and x += alpha y still pending; 2: applied
+  int first;           // first iteration of the step: p = r
+  int force;           // exit tests disabled (tdde_step_forced)
+  int half_iters;      // of the current step
+  int max_half;        // 2 * max_iter
+  int step_idx;        // index into the device g table of the step being solved
+  int pad0;
+  long long steps_done, total_half, applies, preconds;
+  int last_half_iters;
+  int pad1;
+  double last_rel_res;
+};
+
+// finalisation codes: what the last block does with the reduced sums (d0 complex, d1 real)
+enum FinCode {
+  FIN_NONE = 0,
+  FIN_NB,      // nb2 = d1
+  FIN_ALPHA,   // d0 = <rhat, v>  -> alpha = rho / d0
+  FIN_OMEGA,   // d0 = <s, t>, d1 = <t,t>  -> omega = conj(d0) / d1
+  FIN_NORM,    // norm_out = Re d0
+  FIN_R0,      // d0.x = ||b||^2, d1 = ||r0||^2 -> rho, init, zero-iteration exit
+  FIN_S,       // d1 = ||s||^2 -> half-step exit test
+  FIN_R        // d0 = <rhat, r>, d1 = ||r||^2 -> convergence test, rho, beta
+};
+
+struct ReduceCtx {
+  double* partials;        // [TDDE_MAX_PARTIAL_BLOCKS][4]
+  unsigned int* ticket;    // zero between kernels
+  SolverState* st;
+  int fin;
+};
+
+// ---- operator apply ----
+struct ApplyArgs {
+  const cplx* x;           // internal layout
+  cplx* y;
+  const cplx* aux;         // vector for the fused dot (nullable)
+  int n_ang, n_rad, ld;
+  int seg_len;             // radial rows per thread
+  const int* cls;          // [ld] class per channel (pads: class 0)
+  const cplx* blk;         // column-band block coefficients [n_cls][n_rad][2w0+1]: blk[k][j][e] = M_k[j-w0+e][j]
+  cplx beta;               // multiplies every coupling term
+  const double* g;         // device g table
+  const int* step_ptr;     // nullable: row of g = *step_ptr
+  int n_terms;
+  const cplx* Rcol[TDDE_MAX_TERMS];   // column-band [n_rad][2w+1]: Rcol[j][e] = R_L[j-w+e][j]
+  const cplx* Aoff;        // banded path: [n_slots][ld], slot = (term, offset) in kernel order
+  // generic path
+  const int* A_rowptr[TDDE_MAX_TERMS];
+  const int* A_col[TDDE_MAX_TERMS];
+  const cplx* A_val[TDDE_MAX_TERMS];
+  const cplx* Rrow[TDDE_MAX_TERMS];   // row-band [n_rad][2w+1] as at the boundary
+  const cplx* blk_row;     // row-band block coefficients [n_cls][n_rad][2w0+1]
+  int w[TDDE_MAX_TERMS];
+  int w0;
+  int guard;               // 0 none; 1: no-op when st->done|stalled|status (iterations); 2: no-op when stalled|status (start of step)
+  ReduceCtx red;
+};
+
+struct VecArgs {
+  long long n;             // internal element count n_rad * ld
+  cplx *x, *r, *rhat, *p, *v, *s, *t, *y, *z, *b, *u;
+  double dt;               // r0 = -i dt (H c)
+  ReduceCtx red;
+};
+
+struct PrecArgs {
+  const cplx* x;
+  cplx* y;
+  int n_ang, n_rad, ld, w;
+  const int* cls;
+  const cplx* Lcol;        // [n_cls][n_rad][w]:  Lcol[k][i][d-1] = L_k[i+d][i]
+  const cplx* Ucol;        // [n_cls][n_rad][w+1]: Ucol[k][i][0] = 1/U_k[i][i], Ucol[k][i][d] = U_k[i-d][i]
+  const SolverState* st;   // nullable guard
+};
+
+// launchers (each returns the number of kernels launched, or -1 if no instantiation fits)
+int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, cudaStream_t s);
+bool apply_banded_available(int T, int m0, int mstep, int W);
+int launch_apply_generic(const ApplyArgs& a, cudaStream_t s);
+int launch_precond(const PrecArgs& a, cudaStream_t s);
+int launch_vec_r0(const VecArgs& a, cudaStream_t s);
+int launch_vec_p(const VecArgs& a, cudaStream_t s);
+int launch_vec_s(const VecArgs& a, cudaStream_t s);
+int launch_vec_halfexit(const VecArgs& a, cudaStream_t s);
+int launch_vec_xr(const VecArgs& a, cudaStream_t s);
+int launch_step_open(SolverState* st, int step_idx, int force, int clear_stall_only, cudaStream_t s);
+int launch_step_close(SolverState* st, cudaStream_t s);
+int launch_to_internal(const cplx* c, cplx* X, int n_ang, int n_rad, int ld, cudaStream_t s);
+int launch_to_boundary(const cplx* X, cplx* c, int n_ang, int n_rad, int ld, cudaStream_t s);
+int launch_combine_blocks(const cplx* S, const cplx* H0, cplx alpha, cplx beta, cplx* out, long long count, cudaStream_t s);
+int launch_fill(cplx* v, long long n, unsigned seed, cudaStream_t s);
+int launch_dfma_peak(double* out, int blocks, int threads, int iters, cudaStream_t s);

@@ -1,0 +1,115 @@
+"""CPU-side checks of the boundary: libtdde.so builds, loads and exports every symbol include/tdde.h declares;
+the ctypes structs match the header; the product path fails loudly without a GPU (no CPU fallback)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import tdde_inputs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2512_21697_b200.build import build
+    build()
+    import paper_2512_21697_b200 as pkg
+    return pkg.load_library()
+
+
+def header_functions():
+    src = open(os.path.join(ROOT, "include", "tdde.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(tdde_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    import paper_2512_21697_b200 as pkg
+    names = header_functions()
+    assert {"tdde_create", "tdde_step", "tdde_propagate", "tdde_norm", "tdde_apply", "tdde_precond",
+            "tdde_destroy", "tdde_strerror"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), n
+    assert sorted(pkg.EXPORTS) == names
+
+
+def test_struct_layouts_match_header():
+    import paper_2512_21697_b200 as pkg
+    assert C.sizeof(pkg.tdde_config) == 6 * 4 + 2 * 8
+    assert C.sizeof(pkg.tdde_term) == 8 + 4 * 8
+    assert C.sizeof(pkg.tdde_stats) == 4 * 8 + 8 + 2 * 4
+    assert pkg.tdde_config.dt.offset == 24 and pkg.tdde_stats.status.offset == 40
+
+
+def test_strerror_and_version(lib):
+    assert lib.tdde_version() == 1
+    assert lib.tdde_strerror(0) == b"ok"
+    for code in range(-6, 0):
+        assert lib.tdde_strerror(code) not in (b"ok", b"unknown status")
+    assert lib.tdde_strerror(-99) == b"unknown status"
+
+
+def test_create_rejects_bad_arguments_before_touching_cuda(lib):
+    import paper_2512_21697_b200 as pkg
+    p = tdde_inputs.make_config("tiny")
+    h = C.c_void_p()
+    S = np.ascontiguousarray(p.S_band)
+    H0 = np.ascontiguousarray(p.H0_band)
+    cls = np.ascontiguousarray(p.cls_of_chan)
+
+    def cfg(**kw):
+        d = dict(n_ang=p.n_ang, n_rad=p.n_rad, n_cls=p.n_cls, w0=p.w0, n_terms=0, max_iter=10, dt=0.01, rtol=1e-10)
+        d.update(kw)
+        return pkg.tdde_config(d["n_ang"], d["n_rad"], d["n_cls"], d["w0"], d["n_terms"], d["max_iter"], d["dt"], d["rtol"])
+
+    def create(c, cls_arr=cls, S_ptr=None):
+        return lib.tdde_create(C.byref(h), C.byref(c), S.ctypes.data if S_ptr is None else S_ptr, H0.ctypes.data,
+                               cls_arr.ctypes.data, None, None)
+
+    assert create(cfg(n_ang=0)) == -1
+    assert create(cfg(w0=p.n_rad)) == -1
+    assert create(cfg(w0=0)) == -1
+    assert create(cfg(dt=0.0)) == -1
+    assert create(cfg(max_iter=0)) == -1
+    assert create(cfg(n_terms=1)) == -1            # terms pointer is NULL
+    assert create(cfg(n_terms=99)) == -1
+    bad_cls = cls.copy()
+    bad_cls[3] = p.n_cls
+    assert create(cfg(), cls_arr=bad_cls) == -1
+    assert lib.tdde_create(None, C.byref(cfg()), S.ctypes.data, H0.ctypes.data, cls.ctypes.data, None, None) == -1
+    assert h.value is None
+
+
+def test_no_cpu_fallback():
+    """Without a CUDA device the product must refuse to run rather than compute on the host."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    import paper_2512_21697_b200 as pkg
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        pkg.Tdde(tdde_inputs.make_config("tiny"))
+    # and the C ABI itself reports a CUDA error for a valid problem
+    lib = pkg.load_library()
+    p = tdde_inputs.make_config("tiny")
+    c = pkg.tdde_config(p.n_ang, p.n_rad, p.n_cls, p.w0, 0, 10, 0.01, 1e-10)
+    h = C.c_void_p()
+    S = np.ascontiguousarray(p.S_band); H0 = np.ascontiguousarray(p.H0_band); cls = np.ascontiguousarray(p.cls_of_chan)
+    rc = lib.tdde_create(C.byref(h), C.byref(c), S.ctypes.data, H0.ctypes.data, cls.ctypes.data, None, None)
+    assert rc == -3 and h.value is None
+    assert len(lib.tdde_last_cuda_error()) > 0
+
+
+def test_product_does_not_import_oracle():
+    pkg_dir = os.path.join(ROOT, "paper_2512_21697_b200")
+    for dirpath, _, files in os.walk(pkg_dir):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith(".py"):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "paper_2512_21697_b200" not in txt and "libtdde" not in txt, f

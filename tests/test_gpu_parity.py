@@ -1,0 +1,272 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on identical seeded inputs.
+
+Tolerances (BASELINE.json north_star): relative L2 <= 1e-12 per operator apply, <= 1e-9 on the wavefunction
+after a propagation.  Integer results (iteration counts) are compared exactly where both sides are far from
+the tolerance edge, +-1 half-iteration otherwise ("parity unpinned" for counts).
+"""
+import numpy as np
+import pytest
+
+import tdde_inputs
+from oracle import tdde_oracle as orc
+
+pytestmark = pytest.mark.gpu
+
+
+def rel(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def make(name, **kw):
+    from paper_2512_21697_b200 import Tdde
+    p = tdde_inputs.make_config(name, **kw) if isinstance(name, str) else name
+    return p, Tdde(p)
+
+
+def rand_vec(n, seed):
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal(2 * n).view(np.complex128).copy()
+
+
+# a reduced Medium: same structure as BASELINE configs[2] (w = 6, T = 5, offsets 1..L+1), sized for the oracle's CSR
+SMALL_MED = dict(n_ang=100, n_r=150, bandwidth=13, n_terms=5, dt=0.005, n_steps=6, rtol=1e-10, seed=11)
+
+
+@pytest.fixture(scope="module")
+def tiny():
+    p, prop = make("tiny")
+    yield p, prop, orc.assemble(p), orc.factor_precond(p)
+    prop.close()
+
+
+@pytest.fixture(scope="module")
+def tiny_stress():
+    p, prop = make("tiny", phase=np.pi / 2, e0=5.0)
+    yield p, prop, orc.assemble(p), orc.factor_precond(p)
+    prop.close()
+
+
+@pytest.fixture(scope="module")
+def smallmed():
+    from paper_2512_21697_b200 import Tdde
+    p = tdde_inputs.make_synthetic(name="smallmed", phase=np.pi / 2, e0=2.0, **SMALL_MED)
+    prop = Tdde(p)
+    yield p, prop, orc.assemble(p), orc.factor_precond(p)
+    prop.close()
+
+
+@pytest.fixture(scope="module")
+def hyd():
+    from paper_2512_21697_b200 import Tdde
+    p = tdde_inputs.make_hydrogen()
+    prop = Tdde(p)
+    yield p, prop, orc.assemble(p), orc.factor_precond(p)
+    prop.close()
+
+
+def test_paths_selected(tiny, smallmed, hyd):
+    assert tiny[1].apply_path == "banded"
+    assert smallmed[1].apply_path == "banded"
+    assert hyd[1].apply_path == "generic"
+
+
+@pytest.mark.parametrize("which", ["tiny", "smallmed", "hyd"])
+def test_apply_parity(which, request):
+    p, prop, ops, _ = request.getfixturevalue(which)
+    x = rand_vec(p.n, 5)
+    xd = prop.to_device(x)
+    rng = np.random.default_rng(3)
+    for alpha, beta, g in [(1.0, 0.5j * p.dt, p.g_mid(3)), (1.0, -0.5j * p.dt, rng.standard_normal(p.n_terms)),
+                           (0.3 - 0.2j, 1.0 + 0.5j, rng.standard_normal(p.n_terms)), (1.0, 0.0, np.zeros(p.n_terms)),
+                           (0.0, 1.0, np.ones(p.n_terms))]:
+        y = prop.apply(alpha, beta, g, xd).cpu().numpy()
+        y_ref = orc.apply(ops, alpha, beta, np.asarray(g, dtype=float), x)
+        assert rel(y, y_ref) <= 1e-12, (which, alpha, beta)
+
+
+def test_apply_ragged_shapes():
+    """Channel counts that are not multiples of 32/128 and radial sizes that do not divide the segment length."""
+    from paper_2512_21697_b200 import Tdde
+    for n_ang, n_r, T, bw in [(1, 8, 1, 7), (2, 9, 2, 7), (33, 17, 2, 7), (130, 37, 5, 13), (257, 23, 7, 13), (40, 31, 7, 19)]:
+        p = tdde_inputs.make_synthetic(n_ang=n_ang, n_r=n_r, bandwidth=bw, n_terms=T, dt=0.01, n_steps=1, rtol=1e-10,
+                                       seed=n_ang, name="ragged")
+        if n_ang <= T + 1:      # offsets beyond the matrix leave empty terms: must fall back to the generic path
+            pass
+        prop = Tdde(p)
+        ops = orc.assemble(p)
+        x = rand_vec(p.n, 1)
+        g = np.linspace(0.5, 1.5, T)
+        y = prop.apply(1.0, 0.25j, g, prop.to_device(x)).cpu().numpy()
+        assert rel(y, orc.apply(ops, 1.0, 0.25j, g, x)) <= 1e-12, (n_ang, n_r, T, bw, prop.apply_path)
+        z = prop.precond(prop.to_device(x)).cpu().numpy()
+        assert rel(z, orc.apply_precond(orc.factor_precond(p), x)) <= 1e-12, (n_ang, n_r, T, bw)
+        prop.close()
+
+
+@pytest.mark.parametrize("which", ["tiny", "smallmed", "hyd"])
+def test_precond_parity_p8(which, request):
+    p, prop, ops, fact = request.getfixturevalue(which)
+    x = rand_vec(p.n, 7)
+    xd = prop.to_device(x)
+    y = prop.precond(xd).cpu().numpy()
+    assert rel(y, orc.apply_precond(fact, x)) <= 1e-12
+    # M (M^-1 x) = x through tdde_apply with g = 0
+    back = prop.apply(1.0, 0.5j * p.dt, np.zeros(p.n_terms), prop.to_device(y)).cpu().numpy()
+    assert rel(back, x) <= 1e-12
+    # in place
+    prop.precond(xd, xd)
+    assert rel(xd.cpu().numpy(), y) == 0.0
+
+
+@pytest.mark.parametrize("which", ["tiny", "smallmed", "hyd"])
+def test_norm_parity(which, request):
+    p, prop, ops, _ = request.getfixturevalue(which)
+    x = rand_vec(p.n, 9)
+    assert abs(prop.norm(prop.to_device(x)) - orc.s_norm_sq(ops, x)) <= 1e-12 * orc.s_norm_sq(ops, x)
+
+
+@pytest.mark.parametrize("which", ["tiny", "tiny_stress", "smallmed"])
+def test_propagate_parity(which, request):
+    p, prop, ops, fact = request.getfixturevalue(which)
+    n_steps = min(p.n_steps, 10)
+    c_ref, infos = orc.propagate(p, ops, fact, p.c0, n_steps)
+    c = prop.to_device(p.c0)
+    st = prop.propagate(c, p.g_table(n_steps))
+    assert st["steps"] == n_steps and st["status"] == 0
+    assert rel(c.cpu().numpy(), c_ref) <= 1e-9
+    ref_half = sum(i.half_iters for i in infos)
+    assert abs(st["half_iters"] - ref_half) <= n_steps, (st, ref_half)     # +-1 half-iteration per step at the edge
+    assert st["rel_res"] <= p.rtol
+    assert abs(prop.norm(c) - 1.0) <= 10 * n_steps * p.rtol                 # P2 on the GPU path
+
+
+def test_step_equals_propagate_of_one(tiny_stress):
+    p, prop, ops, fact = tiny_stress
+    c1 = prop.to_device(p.c0)
+    c2 = prop.to_device(p.c0)
+    for s in range(3):
+        prop.step(c1, p.g_mid(s))
+    prop.propagate(c2, p.g_table(3))
+    assert np.array_equal(c1.cpu().numpy(), c2.cpu().numpy())
+
+
+def test_hydrogen_field_free_and_field(hyd):
+    p, prop, ops, fact = hyd
+    # field-free: exact preconditioner => the ||s|| exit at half-iteration 1 every step (C8-11, P3)
+    c = prop.to_device(p.c0)
+    g0 = np.zeros((5, p.n_terms))
+    st = prop.propagate(c, g0)
+    assert st["half_iters"] == 5 and st["steps"] == 5
+    pz = tdde_inputs.Problem(**{**p.__dict__, "g_of_t": lambda t: np.zeros(p.n_terms)})
+    c_ref, _ = orc.propagate(pz, ops, fact, p.c0, 5)
+    assert rel(c.cpu().numpy(), c_ref) <= 1e-9
+    # under the field
+    c = prop.to_device(p.c0)
+    n_steps = 5
+    first = 40
+    gt = p.g_table(n_steps, first_step=first)
+    st = prop.propagate(c, gt)
+    c_ref, infos = orc.propagate(p, ops, fact, p.c0, n_steps, first_step=first)
+    assert rel(c.cpu().numpy(), c_ref) <= 1e-9
+    assert abs(prop.norm(c) - orc.s_norm_sq(ops, p.c0)) <= 1e-9
+
+
+def test_fixed_iteration_trace_p11(tiny_stress):
+    p, prop, ops, fact = tiny_stress
+    k = 4
+    g = p.g_mid(0)
+    x_ref, info = orc.cn_step(ops, fact, p.c0, g, p.dt, p.rtol, p.max_iter, force_iters=k, keep_trace=True)
+    c = prop.to_device(p.c0)
+    tr = prop.step_forced(c, g, k).cpu().numpy()
+    names = ["p", "v", "s", "t", "x", "r", "y", "z"]
+    for it in range(k):
+        for q, nm in enumerate(names):
+            ref = info.trace[it][nm]
+            scale = max(np.linalg.norm(ref), 1e-300)
+            # residual-like vectors shrink by orders of magnitude per iteration: compare against ||b||-scaled floor
+            tol = 1e-11 * max(1.0, np.linalg.norm(info.trace[0]["p"]) / scale) if nm in ("s", "r", "t", "v", "p", "y", "z") else 1e-11
+            assert np.linalg.norm(tr[it, q] - ref) / scale <= min(tol, 1e-6), (it, nm)
+    assert rel(c.cpu().numpy(), x_ref) <= 1e-11
+
+
+def test_determinism_p12(smallmed):
+    p, prop, _, _ = smallmed
+    outs = []
+    for _ in range(2):
+        c = prop.to_device(p.c0)
+        prop.propagate(c, p.g_table(4))
+        outs.append(c.cpu().numpy().copy())
+    assert np.array_equal(outs[0], outs[1])
+
+
+def test_speculation_stall_and_resume():
+    """A hard system (strong field) needs more iterations than are speculated per step: the stall latch, the
+    resume path and the growth of nspec must give the same answer as the oracle."""
+    p, prop = make("tiny", phase=np.pi / 2, e0=40.0)
+    ops, fact = orc.assemble(p), orc.factor_precond(p)
+    c_ref, infos = orc.propagate(p, ops, fact, p.c0, 4)
+    assert max(i.half_iters for i in infos) > 6
+    c = prop.to_device(p.c0)
+    st = prop.propagate(c, p.g_table(4))
+    assert st["steps"] == 4
+    assert rel(c.cpu().numpy(), c_ref) <= 1e-9
+    prop.close()
+
+
+def test_noconv_is_reported():
+    p, prop = make("tiny", phase=np.pi / 2, e0=40.0, max_iter=1)
+    c = prop.to_device(p.c0)
+    st = prop.propagate(c, p.g_table(2), check=False)
+    assert st["rc"] == -6 and st["status"] == -6 and st["steps"] == 0
+    # the handle stays usable: field-free steps converge at once
+    st = prop.propagate(c, np.zeros((2, p.n_terms)))
+    assert st["steps"] == 2
+    prop.close()
+
+
+def test_time_reversal_p4(tiny_stress):
+    from paper_2512_21697_b200 import Tdde
+    p, prop, _, _ = tiny_stress
+    back = Tdde(p, dt=-p.dt)
+    c = prop.to_device(p.c0)
+    g = p.g_mid(2)
+    prop.step(c, g)
+    back.step(c, g)
+    assert rel(c.cpu().numpy(), p.c0) <= 10 * p.rtol
+    back.close()
+
+
+def test_propagate_host_roundtrip(tiny_stress):
+    p, prop, ops, fact = tiny_stress
+    c = p.c0.copy()
+    prop.propagate_host(c, p.g_table(3), 3)
+    d = prop.to_device(p.c0)
+    prop.propagate(d, p.g_table(3))
+    assert np.array_equal(c, d.cpu().numpy())
+
+
+def test_sampled_rows_at_bench_size_p10():
+    """BASELINE configs[3] (Large) in the launch configuration bench.py times: sampled outputs against the
+    oracle's direct summation of the definition (the CSR would need 17 GB)."""
+    p, prop = make("large", with_c0=False)
+    assert prop.apply_path == "banded"
+    import torch
+    x = rand_vec(p.n, 21)
+    xd = prop.to_device(x)
+    g = np.linspace(-1.0, 1.0, p.n_terms)
+    y = prop.apply(1.0, 0.5j * p.dt, g, xd).cpu().numpy().reshape(p.n_ang, p.n_rad)
+    rng = np.random.default_rng(0)
+    ns = 400
+    chan = np.concatenate([rng.integers(0, p.n_ang, ns), [0, 0, p.n_ang - 1, p.n_ang - 1, 1, 5, p.n_ang - 6]])
+    rad = np.concatenate([rng.integers(0, p.n_rad, ns), [0, p.n_rad - 1, 0, p.n_rad - 1, 5, 6, p.n_rad - 7]])
+    ref = orc.apply_rows_sampled(p, 1.0, 0.5j * p.dt, g, x, chan, rad)
+    got = y[chan, rad]
+    scale = np.sqrt(np.mean(np.abs(ref) ** 2))
+    assert np.max(np.abs(got - ref)) / scale <= 1e-12
+    # properties that hold at any size: M (M^-1 x) = x, and S-norm of a normalised vector
+    z = prop.precond(xd)
+    back = prop.apply(1.0, 0.5j * p.dt, np.zeros(p.n_terms), z).cpu().numpy()
+    assert rel(back, x) <= 1e-12
+    del xd, z
+    torch.cuda.empty_cache()
+    prop.close()
