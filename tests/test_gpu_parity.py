@@ -58,7 +58,14 @@ def smallmed():
 @pytest.fixture(scope="module")
 def hyd():
     from paper_2512_21697_b200 import Tdde
+    import scipy.linalg as sla
     p = tdde_inputs.make_hydrogen()
+    # c0 = the 1s1/2 (kappa = -1, mu = +1/2) eigenstate of the field-free block, S-normalised by eigh
+    S, H = p.meta["dense"][-1]
+    E, V = sla.eigh(H, S)
+    j = int(np.nonzero(E > -p.meta["c"] ** 2)[0][0])
+    a = p.meta["chans"].index((-1, 0.5))
+    p.c0[a * p.n_rad:(a + 1) * p.n_rad] = V[:, j]
     prop = Tdde(p)
     yield p, prop, orc.assemble(p), orc.factor_precond(p)
     prop.close()
