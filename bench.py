@@ -1,0 +1,275 @@
+#!/usr/bin/env python
+"""bench.py -- CN time steps/s (and BiCGSTAB iterations/s, operator applies/s) of the TDDE propagator on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config hbm|large|medium|...] [--impl ours|reference]
+
+One "step" is one Crank-Nicolson step = one pass of the whole hot path (two start-of-step applies, the BiCGSTAB
+iterations with their preconditioner solves, fused vector kernels and on-device scalar updates).
+The default workload is BASELINE.json's HBM-scale synthetic config, the largest single-GPU configuration
+(vectors of 512 MB: every pass is larger than the 126 MB L2, so no L2 flush is needed between steps).
+Prints ONE JSON line (see DESIGN.md "Measurement" for every field).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import tdde_inputs  # noqa: E402
+
+METRIC = "cn_time_steps_per_s"
+UNIT = "steps/s"
+NUM_SMS = 148
+FP64_FMA_PER_CLK_PER_SM = 64          # B200: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2 TFLOP/s nominal
+
+
+def f_apply(p) -> int:
+    """Complex FMAs per vector element of one operator apply: n_d + sum_L (n_d + nnz_row(A_L))."""
+    nd = 2 * p.w0 + 1
+    tot = nd
+    for t in p.terms:
+        nnz_row = int(np.max(np.diff(t.A_rowptr)))       # interior rows
+        tot += (2 * t.w + 1) + nnz_row
+    return tot
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag, self.max_mhz = index, [], set(), False, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap"}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(0.05)
+
+    def result(self):
+        self.stop_flag = True
+        if self.nv is None or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
+
+
+# ----------------------------------------------------------------------------------------------- reference arm
+def oracle_sample_problem(cfg_name: str, sample_ang: int):
+    """The same workload recipe restricted to `sample_ang` angular channels (all radial sizes, bandwidth, terms kept)."""
+    args = dict(tdde_inputs.CONFIGS[cfg_name])
+    full_n = args["n_ang"] * 2 * args["n_r"]
+    args["n_ang"] = min(sample_ang, args["n_ang"])
+    p = tdde_inputs.make_synthetic(name=cfg_name + "-sample", **args)
+    return p, full_n
+
+
+def run_oracle(cfg_name: str, steps: int, warmup: int, sample_ang: int):
+    """Times the CPU oracle as it stands (SciPy CSR + textbook BiCGSTAB, one thread) on a bounded sample."""
+    from oracle import tdde_oracle as orc
+    p, full_n = oracle_sample_problem(cfg_name, sample_ang)
+    ops = orc.assemble(p)
+    fact = orc.factor_precond(p)
+    c = p.c0.copy()
+    if warmup:
+        c, _ = orc.propagate(p, ops, fact, c, warmup, first_step=0)
+    t0 = time.perf_counter()
+    c, infos = orc.propagate(p, ops, fact, c, steps, first_step=warmup)
+    dt = time.perf_counter() - t0
+    sample_steps_per_s = steps / dt
+    scaled = sample_steps_per_s * p.n / full_n
+    return dict(value=scaled, unit=UNIT, cores=1, kind="oracle",
+                sample=f"{cfg_name} recipe cut to {p.n_ang} of {tdde_inputs.CONFIGS[cfg_name]['n_ang']} angular channels "
+                       f"(n={p.n}), {steps} CN steps in {dt:.2f} s; value = sample steps/s x n_sample/n_full",
+                half_iters=int(sum(i.half_iters for i in infos)), seconds=dt), p
+
+
+def reference_main(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    steps = max(1, min(args.steps, 4))
+    cb, p = run_oracle(args.config, steps, min(args.warmup, 1), args.sample_ang)
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / cb["value"], "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)", "data": "synthetic",
+            "config": {"workload": args.config, "note": "CPU oracle on a bounded sample, scaled to the full workload"},
+            "cpu_baseline": {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------------------------------- our arm
+def ours_main(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2512_21697_b200 import Tdde
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    K, W = args.steps, max(args.warmup, 3)
+    p = tdde_inputs.make_config(args.config, phase=args.phase)
+    prop = Tdde(p, device=f"cuda:{local}")
+    g_all = p.g_table(W + K)
+    c = prop.to_device(p.c0)
+    n, T = p.n, p.n_terms
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: W warm-up steps, then exactly K steps ----
+    prop.propagate(c, g_all[:W])
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    launches0 = prop.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    st = prop.propagate(c, g_all[W:W + K])
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    launches = prop.launch_count - launches0
+    norm_end = prop.norm(c)
+
+    # ---- per-kernel timings, live, CUDA events on the handle's stream (same process, right after) ----
+    g_mid = g_all[W]
+    reps = args.kernel_reps
+    kt = {name: prop.time_kernel(which, reps, g_mid) for which, name in
+          [(0, "apply"), (1, "precond"), (2, "vec_p"), (3, "vec_s"), (4, "vec_xr"), (5, "transpose"), (6, "apply_S")]}
+    fp64_peak_meas = prop.fp64_peak()
+    clocks = sampler.result()
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
+    c_host_t = torch.empty(n, dtype=torch.complex128).pin_memory()
+    c_host = c_host_t.numpy()
+    c_host[:] = p.c0
+    prop.propagate_host(c_host, g_all[:W], W)              # warm-up (allocates the staging buffer)
+    barrier()
+    t0 = time.perf_counter()
+    prop.propagate_host(c_host, g_all[W:W + K], K)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+
+    if world > 1:
+        t = torch.tensor([ms, e2e_s * 1e3], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, e2e_ms = float(t[0]), float(t[1])
+    else:
+        e2e_ms = e2e_s * 1e3
+
+    if rank == 0:
+        peaks, peak_kind = load_peaks()
+        F = f_apply(p)
+        nint = n                                            # algorithmic element count (pads excluded)
+        flops_apply = 8.0 * F * nint
+        sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+        fp64_peak_nominal = NUM_SMS * FP64_FMA_PER_CLK_PER_SM * 2 * sm_max * 1e6
+        t_apply = kt["apply"] * 1e-3
+        ach = flops_apply / t_apply / 1e12
+        hbm = float(peaks["hbm_gbs"])
+        bytes_per = {"apply": 48, "precond": 32, "vec_p": 64, "vec_s": 48, "vec_xr": 128, "transpose": 32, "apply_S": 32}
+        kernels = {k: {"ms": v, "alg_GBps": bytes_per[k] * nint / (v * 1e-3) / 1e9,
+                       "hbm_frac": bytes_per[k] * nint / (v * 1e-3) / 1e9 / hbm} for k, v in kt.items()}
+        steps_per_s = world * K / (ms * 1e-3)
+        line = {
+            "metric": METRIC, "value": steps_per_s, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "complex128 (f64)", "data": "synthetic",
+            "config": {"workload": args.config, "n_ang": p.n_ang, "n_rad": p.n_rad, "n": n, "bandwidth": 2 * p.w0 + 1,
+                       "n_terms": T, "dt": p.dt, "rtol": p.rtol, "seed": p.seed, "phase": args.phase,
+                       "apply_path": prop.apply_path, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "l2": "vectors (%.0f MB each) exceed the 126 MB L2; no flush" % (n * 16 / 1e6)},
+            "bicgstab_iters_per_s": world * 0.5 * st["half_iters"] / (ms * 1e-3),
+            "applies_per_s": world * st["applies"] / (ms * 1e-3),
+            "half_iters_per_step": st["half_iters"] / K, "rel_res": st["rel_res"], "s_norm_end": norm_end,
+            "gpu_launches": launches,
+            "clocks": clocks,
+            "e2e": {"value": world * K / (e2e_ms * 1e-3), "unit": UNIT,
+                    "h2d_bytes_per_step": (n * 16 + K * T * 8) / K, "d2h_bytes_per_step": n * 16 / K,
+                    "note": "one tdde_propagate_host call of K steps: state vector H2D + g table H2D + K steps + state D2H"},
+            "roofline": {"bound": "alu", "kernel": "k_apply_banded (v = A y with fused <rhat,v>)",
+                         "achieved": ach, "peak": fp64_peak_nominal / 1e12, "unit": "TFLOP/s",
+                         "frac": ach / (fp64_peak_nominal / 1e12), "traffic": None,
+                         "peak_kind": "derived: 148 SMs x 64 DFMA/clk x 2 x %.0f MHz" % sm_max,
+                         "fp64_peak_measured_tflops": fp64_peak_meas / 1e12,
+                         "frac_of_measured_dfma": ach / (fp64_peak_meas / 1e12),
+                         "cfma_per_element": F, "flops_per_launch": flops_apply,
+                         "alg_hbm_GBps": kernels["apply"]["alg_GBps"], "hbm_peak_GBps": hbm, "hbm_peak_kind": peak_kind},
+            "kernels": kernels,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            cb, _ = run_oracle(args.config, 2, 0, args.sample_ang)
+            line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        print(json.dumps(line))
+    prop.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="hbm", choices=sorted(tdde_inputs.CONFIGS))
+    ap.add_argument("--phase", type=float, default=0.0, help="phase of g(t) = E0 sin(w t + phase); 0 = BASELINE config")
+    ap.add_argument("--kernel-reps", type=int, default=10)
+    ap.add_argument("--sample-ang", type=int, default=12, help="angular channels of the oracle's bounded sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        reference_main(args)
+    else:
+        ours_main(args)
+
+
+if __name__ == "__main__":
+    main()

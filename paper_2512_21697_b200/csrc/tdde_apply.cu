@@ -17,6 +17,8 @@
 #include "tdde_reduce.cuh"
 
 #define AP_NT 128
+#define AP_JC TDDE_AP_JC      // radial rows per pipeline stage
+#define AP_MAXC TDDE_AP_MAXC  // distinct kappa-classes per CTA staged in shared memory
 
 template <int T, int M0, int MS>
 struct BandShape {
@@ -30,21 +32,112 @@ struct BandShape {
   __host__ __device__ static constexpr int nslots() { return slot0(T); }
 };
 
+// ---- TMA (1-D bulk async copy) + mbarrier helpers: raw PTX, sm_90+ ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+               "l"(src), "r"(bytes), "r"(smem_u32(bar))
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok)
+                 : "r"(smem_u32(bar)), "r"(parity)
+                 : "memory");
+  } while (!ok);
+}
+
+// Shared-memory plan of one pipeline stage (JC radial rows):
+//   Rs[JC][T][ND]     radial column coefficients of every term (one bulk copy: host stores them [n_rad][T][ND])
+//   Bs[MAXC][JC][ND]  block column coefficients of the (at most MAXC) distinct kappa-classes of this CTA
+//   Xs[JC][XW]        x rows of the CTA's 128 channels plus MAXM halo channels on each side (one bulk copy per row)
 template <int T, int M0, int MS, int W>
-__global__ void __launch_bounds__(AP_NT) k_apply_banded(const ApplyArgs p) {
+struct ApplyPlan {
   using SH = BandShape<T, M0, MS>;
-  constexpr int ND = 2 * W + 1;
-  constexpr int MAXM = SH::maxm();
-  constexpr int NS = SH::nslots();
+  static constexpr int ND = 2 * W + 1;
+  static constexpr int MAXM = SH::maxm();
+  static constexpr int XW = AP_NT + 2 * MAXM;
+  static constexpr int RS = AP_JC * T * ND;                 // complex elements
+  static constexpr int BS = AP_MAXC * AP_JC * ND;
+  static constexpr int XS = AP_JC * XW;
+  static constexpr int STAGE = RS + BS + XS;
+  static constexpr size_t SMEM = (size_t)2 * STAGE * sizeof(cplx) + 64;
+};
+
+template <int T, int M0, int MS, int W>
+__global__ void __launch_bounds__(AP_NT, 2) k_apply_banded(const ApplyArgs p) {
+  using SH = BandShape<T, M0, MS>;
+  using PL = ApplyPlan<T, M0, MS, W>;
+  constexpr int ND = PL::ND, MAXM = PL::MAXM, NS = SH::nslots(), XW = PL::XW, JC = AP_JC;
   if (p.guard == 1 && solver_idle(p.red.st)) return;
   if (p.guard == 2 && (p.red.st->stalled | (p.red.st->status != 0))) return;
 
-  const int a = blockIdx.x * AP_NT + threadIdx.x;         // channel (may be a pad lane: a < ld always)
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  cplx* stage_base = reinterpret_cast<cplx*>(smem_raw);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)2 * PL::STAGE * sizeof(cplx));
+
+  const int tid = threadIdx.x;
+  const int a0 = blockIdx.x * AP_NT;
+  const int a = a0 + tid;                                   // channel; lanes with a >= ld idle along
   const int ld = p.ld, n_rad = p.n_rad;
   const bool lane_ok = a < ld;
   const int ac = lane_ok ? a : ld - 1;
   const int i0 = blockIdx.y * p.seg_len;
   const int i1 = min(n_rad, i0 + p.seg_len);
+  const int jlo = max(0, i0 - W), jhi = min(n_rad, i1 + W);   // input rows this segment needs
+  const int nchunks = (jhi - jlo + JC - 1) / JC;
+
+  // channel range of the x tile, clipped to the vector; the clipped cells stay zero (matching A entries are 0)
+  const int xa_lo = max(0, a0 - MAXM), xa_hi = min(ld, a0 + AP_NT + MAXM);
+  const int x_dst_off = xa_lo - (a0 - MAXM);
+  const uint32_t x_bytes = (uint32_t)(xa_hi - xa_lo) * sizeof(cplx);
+  const int* cta_cls = p.cta_cls + blockIdx.x * AP_MAXC;
+
+  if (x_bytes != XW * sizeof(cplx)) {
+    for (int q = tid; q < 2 * PL::STAGE; q += AP_NT) stage_base[q] = make_double2(0, 0);
+  }
+  if (tid == 0) {
+    mbar_init(&full[0], 1);
+    mbar_init(&full[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+
+  auto issue = [&](int c) {                                  // one elected thread: all bulk copies of chunk c
+    cplx* st = stage_base + (size_t)(c & 1) * PL::STAGE;
+    uint64_t* bar = &full[c & 1];
+    const int j = jlo + c * JC;
+    const int nr = min(JC, jhi - j);
+    uint32_t bytes = (uint32_t)nr * x_bytes;
+    int ncls = 0;
+#pragma unroll
+    for (int q = 0; q < AP_MAXC; ++q) ncls += (cta_cls[q] >= 0);
+    bytes += (uint32_t)ncls * nr * ND * sizeof(cplx);
+    if (T > 0) bytes += (uint32_t)nr * T * ND * sizeof(cplx);
+    mbar_expect_tx(bar, bytes);
+    if (T > 0) bulk_g2s(st, p.Rall + (size_t)j * T * ND, (uint32_t)nr * T * ND * sizeof(cplx), bar);
+#pragma unroll
+    for (int q = 0; q < AP_MAXC; ++q) {
+      const int k = cta_cls[q];
+      if (k >= 0)
+        bulk_g2s(st + PL::RS + (size_t)q * JC * ND, p.blk + ((size_t)k * n_rad + j) * ND, (uint32_t)nr * ND * sizeof(cplx), bar);
+    }
+    for (int r = 0; r < nr; ++r)
+      bulk_g2s(st + PL::RS + PL::BS + (size_t)r * XW + x_dst_off, p.x + (size_t)(j + r) * ld + xa_lo, x_bytes, bar);
+  };
+  if (tid == 0) {
+    issue(0);
+    if (nchunks > 1) issue(1);
+  }
 
   // angular coefficients in registers, pre-multiplied by beta * g_L
   cplx Areg[NS > 0 ? NS : 1];
@@ -61,8 +154,8 @@ __global__ void __launch_bounds__(AP_NT) k_apply_banded(const ApplyArgs p) {
       }
     }
   }
-  const int k = p.cls[ac];
-  const cplx* blk = p.blk + (size_t)k * n_rad * ND;
+  const int slot = p.slot[ac];                               // index into this CTA's class list, or -1
+  const cplx* blk_g = p.blk + (size_t)p.cls[ac] * n_rad * ND;   // global fallback for slot < 0
 
   cplx yw[ND];
 #pragma unroll
@@ -70,14 +163,28 @@ __global__ void __launch_bounds__(AP_NT) k_apply_banded(const ApplyArgs p) {
   cplx d0 = make_double2(0, 0);
   double d1 = 0;
 
-  for (int j = i0 - W; j < i1 + W; ++j) {
-    if (j >= 0 && j < n_rad) {
-      const cplx* xr = p.x + (size_t)j * ld;
-      const cplx x0 = xr[ac];
-      // block part: per-lane class coefficients
-      const cplx* bc = blk + (size_t)j * ND;
+  for (int c = 0; c < nchunks; ++c) {
+    const cplx* st = stage_base + (size_t)(c & 1) * PL::STAGE;
+    mbar_wait(&full[c & 1], (c >> 1) & 1);
+    const int jc0 = jlo + c * JC;
+    const int nr = min(JC, jhi - jc0);
+    for (int r = 0; r < nr; ++r) {
+      const int j = jc0 + r;
+      const int i = j - W;                                   // the output row completed by input row j
+      const bool emit = (i >= i0) && lane_ok;                // i < i1 always holds here
+      cplx ax = make_double2(0, 0);
+      if (emit && p.aux) ax = p.aux[(size_t)i * ld + a];
+      const cplx* xs = st + PL::RS + PL::BS + (size_t)r * XW + tid + MAXM;
+      const cplx x0 = xs[0];
+      if (slot >= 0) {
+        const cplx* bc = st + PL::RS + ((size_t)slot * JC + r) * ND;
 #pragma unroll
-      for (int e = 0; e < ND; ++e) cfma(yw[e], __ldg(bc + e), x0);
+        for (int e = 0; e < ND; ++e) cfma(yw[e], bc[e], x0);
+      } else {
+        const cplx* bc = blk_g + (size_t)j * ND;
+#pragma unroll
+        for (int e = 0; e < ND; ++e) cfma(yw[e], __ldg(bc + e), x0);
+      }
       if (T > 0) {
         cplx z[T > 0 ? T : 1];
 #pragma unroll
@@ -85,8 +192,7 @@ __global__ void __launch_bounds__(AP_NT) k_apply_banded(const ApplyArgs p) {
 #pragma unroll
         for (int o = -MAXM; o <= MAXM; ++o) {
           if (o == 0) continue;
-          const int ao = min(max(ac + o, 0), ld - 1);      // clamped: the matching A entry is 0 there
-          const cplx xo = xr[ao];
+          const cplx xo = xs[o];
 #pragma unroll
           for (int L = 0; L < T; ++L) {
             if (SH::m(L) >= (o < 0 ? -o : o)) {
@@ -98,21 +204,31 @@ __global__ void __launch_bounds__(AP_NT) k_apply_banded(const ApplyArgs p) {
         }
 #pragma unroll
         for (int L = 0; L < T; ++L) {
-          const cplx* rc = p.Rcol[L] + (size_t)j * ND;      // warp-uniform address
+          const cplx* rc = st + ((size_t)r * T + L) * ND;    // warp-uniform: broadcast LDS.128
 #pragma unroll
-          for (int e = 0; e < ND; ++e) cfma(yw[e], __ldg(rc + e), z[L]);
+          for (int e = 0; e < ND; ++e) cfma(yw[e], rc[e], z[L]);
         }
       }
+      if (emit) {
+        const cplx yv = yw[0];
+        p.y[(size_t)i * ld + a] = yv;
+        cfma_conj(d0, ax, yv);
+        d1 = fma(yv.x, yv.x, d1); d1 = fma(yv.y, yv.y, d1);
+      }
+#pragma unroll
+      for (int e = 0; e < ND - 1; ++e) yw[e] = yw[e + 1];
+      yw[ND - 1] = make_double2(0, 0);
     }
-    // row i = j - W is complete
+    __syncthreads();                                         // every warp is done with this stage
+    if (tid == 0 && c + 2 < nchunks) issue(c + 2);
+  }
+  // rows past the end of the matrix contribute nothing: flush the outputs still in the window
+  for (int j = jhi; j < i1 + W; ++j) {
     const int i = j - W;
-    if (i >= i0 && i < i1 && lane_ok) {
+    if (i >= i0 && lane_ok) {
       const cplx yv = yw[0];
       p.y[(size_t)i * ld + a] = yv;
-      if (p.aux) {
-        const cplx ax = p.aux[(size_t)i * ld + a];
-        cfma_conj(d0, ax, yv);
-      }
+      if (p.aux) cfma_conj(d0, p.aux[(size_t)i * ld + a], yv);
       d1 = fma(yv.x, yv.x, d1); d1 = fma(yv.y, yv.y, d1);
     }
 #pragma unroll
@@ -184,7 +300,17 @@ bool apply_banded_available(int T, int m0, int mstep, int W) {
 int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, cudaStream_t s) {
   dim3 grid((a.ld + AP_NT - 1) / AP_NT, (a.n_rad + a.seg_len - 1) / a.seg_len);
 #define X(t, aa, b, w) \
-  if (T == t && (t == 0 || (m0 == aa && mstep == b)) && W == w) { k_apply_banded<t, aa, b, w><<<grid, AP_NT, 0, s>>>(a); return 1; }
+  if (T == t && (t == 0 || (m0 == aa && mstep == b)) && W == w) {                                         \
+    static bool attr_set = false;                                                                         \
+    const size_t smem = ApplyPlan<t, aa, b, w>::SMEM;                                                     \
+    if (!attr_set) {                                                                                      \
+      if (cudaFuncSetAttribute(k_apply_banded<t, aa, b, w>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
+                               (int)smem) != cudaSuccess) return -2;                                      \
+      attr_set = true;                                                                                    \
+    }                                                                                                     \
+    k_apply_banded<t, aa, b, w><<<grid, AP_NT, smem, s>>>(a);                                             \
+    return 1;                                                                                             \
+  }
   TDDE_BANDED_SHAPES(X)
 #undef X
   return -1;

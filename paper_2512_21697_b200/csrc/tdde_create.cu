@@ -119,7 +119,7 @@ bool detect_banded(const tdde_config* c, const tdde_term* terms, int* m0, int* m
 extern "C" void tdde_destroy(tdde_handle* h) {
   if (!h) return;
   cudaStreamSynchronize(h->stream);
-  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Lcol, h->d_Ucol, h->X, h->r,
+  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_Lcol, h->d_Ucol, h->X, h->r,
                   h->rhat, h->p, h->v, h->s, h->t, h->y, h->z, h->c_stage, h->d_st, h->d_st_bench, h->d_partials,
                   h->d_ticket, h->d_g, h->d_g_small, h->d_zero_g};
   for (void* p : ptrs) if (p) cudaFree(p);
@@ -150,14 +150,23 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
   h->bT = T; h->bM0 = m0; h->bMS = ms; h->bW = w0;
   h->norm_banded = (h->path == 1);
 
-  // radial segment length: enough thread blocks to fill 148 SMs several times, yet long enough that the
-  // 2W halo rows recomputed per segment stay a small fraction
+  // radial segment length (banded path): the kernel runs 2 CTAs per SM (296 slots on 148 SMs); every segment
+  // recomputes 2 w0 halo rows.  Pick the segment count that minimises waves x (rows + halo).
   {
     const int chan_blocks = (h->ld + 127) / 128;
-    int want_segs = (148 * 4 + chan_blocks - 1) / chan_blocks;
-    int seg = (n_rad + want_segs - 1) / want_segs;
-    seg = std::max(seg, 4 * w0);
-    h->seg_len = std::min(seg, n_rad);
+    const int slots = 148 * 2;
+    long long best_cost = -1;
+    int best_seg = n_rad;
+    for (int segs = 1; segs <= n_rad; ++segs) {
+      const int seg = (n_rad + segs - 1) / segs;
+      if (seg < 2 * w0 && segs > 1) break;
+      const int real_segs = (n_rad + seg - 1) / seg;
+      const long long ctas = (long long)chan_blocks * real_segs;
+      const long long waves = (ctas + slots - 1) / slots;
+      const long long cost = waves * (seg + 2 * w0);
+      if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_seg = seg; }
+    }
+    h->seg_len = best_seg;
   }
 
   const zc* S = reinterpret_cast<const zc*>(S_band);
@@ -228,16 +237,42 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     if (rc) return rc;
     CU(cudaStreamSynchronize(s));
   }
-  for (int L = 0; L < T; ++L) {
+  if (h->path == 1) {
+    // per CTA (128 consecutive channels): the first TDDE_AP_MAXC distinct classes are staged in shared memory
+    const int n_cta = (h->ld + 127) / 128;
+    std::vector<int> slot(h->ld, -1), cta_cls((size_t)n_cta * TDDE_AP_MAXC, -1);
+    for (int b = 0; b < n_cta; ++b) {
+      int cnt = 0;
+      for (int a = b * 128; a < std::min(h->ld, (b + 1) * 128); ++a) {
+        const int k = a < c.n_ang ? cls_of_chan[a] : 0;
+        int q = 0;
+        while (q < cnt && cta_cls[(size_t)b * TDDE_AP_MAXC + q] != k) ++q;
+        if (q == cnt && cnt < TDDE_AP_MAXC) cta_cls[(size_t)b * TDDE_AP_MAXC + cnt++] = k;
+        slot[a] = q < cnt ? q : -1;
+      }
+    }
+    int rc;
+    if ((rc = dev_upload(&h->d_slot, slot.data(), slot.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_cta_cls, cta_cls.data(), cta_cls.size(), s))) return rc;
+    const int nd = 2 * w0 + 1;
+    std::vector<zc> Rall((size_t)n_rad * std::max(T, 1) * nd), Rc((size_t)n_rad * nd);
+    for (int L = 0; L < T; ++L) {
+      row_to_col_band(reinterpret_cast<const zc*>(terms[L].R_band), Rc.data(), n_rad, w0);
+      for (int j = 0; j < n_rad; ++j)
+        std::memcpy(&Rall[((size_t)j * T + L) * nd], &Rc[(size_t)j * nd], nd * sizeof(zc));
+    }
+    if ((rc = dev_upload(&h->d_Rall, reinterpret_cast<cplx*>(Rall.data()), Rall.size(), s))) return rc;
+    CU(cudaStreamSynchronize(s));
+  }
+  for (int L = 0; L < T && h->path == 0; ++L) {
     const int w = terms[L].w, nd = 2 * w + 1;
     h->w[L] = w;
     const zc* R = reinterpret_cast<const zc*>(terms[L].R_band);
     std::vector<zc> Rx((size_t)n_rad * nd);
-    if (h->path == 1) row_to_col_band(R, Rx.data(), n_rad, w);
-    else std::memcpy(Rx.data(), R, Rx.size() * sizeof(zc));
+    std::memcpy(Rx.data(), R, Rx.size() * sizeof(zc));
     int rc;
     if ((rc = dev_upload(&h->d_R[L], reinterpret_cast<cplx*>(Rx.data()), Rx.size(), s))) return rc;
-    if (h->path == 0) {
+    {
       const int nnz = terms[L].A_rowptr[c.n_ang];
       std::vector<int> rp(h->ld + 1, nnz);
       for (int a = 0; a <= c.n_ang; ++a) rp[a] = terms[L].A_rowptr[a];

@@ -38,7 +38,7 @@ int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int b
   const bool banded = (h->path == 1);
   if (banded) {
     a.blk = blk_ptr(h, blk);
-    for (int L = 0; L < T; ++L) a.Rcol[L] = h->d_R[L];
+    a.Rall = h->d_Rall; a.slot = h->d_slot; a.cta_cls = h->d_cta_cls;
     a.Aoff = h->d_Aoff;
     rc = launch_apply_banded(a, T, h->bM0, h->bMS, h->cfg.w0, h->stream);
   } else {
@@ -49,6 +49,7 @@ int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int b
     }
     rc = launch_apply_generic(a, h->stream);
   }
+  if (rc == -2) return tdde_cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(apply)");
   if (rc < 0) return TDDE_EINVAL;
   h->launches += rc;
   return 0;

@@ -28,6 +28,8 @@ struct tdde_handle {
   cplx* d_R[TDDE_MAX_TERMS] = {};            // per term band in the path's layout (col-band or row-band)
   int w[TDDE_MAX_TERMS] = {};
   cplx* d_Aoff = nullptr;                    // banded path
+  cplx* d_Rall = nullptr;                    // banded path: [n_rad][T][2w+1]
+  int *d_slot = nullptr, *d_cta_cls = nullptr;
   int* d_Arowptr[TDDE_MAX_TERMS] = {};       // generic path
   int* d_Acol[TDDE_MAX_TERMS] = {};
   cplx* d_Aval[TDDE_MAX_TERMS] = {};

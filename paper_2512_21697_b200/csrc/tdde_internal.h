@@ -13,6 +13,8 @@
 #define TDDE_MAX_TERMS 8
 #define TDDE_MAX_PARTIAL_BLOCKS 65536
 #define TDDE_TINY 1e-290
+#define TDDE_AP_JC 8
+#define TDDE_AP_MAXC 4
 
 typedef double2 cplx;
 
@@ -71,7 +73,9 @@ struct ApplyArgs {
   const double* g;         // device g table
   const int* step_ptr;     // nullable: row of g = *step_ptr
   int n_terms;
-  const cplx* Rcol[TDDE_MAX_TERMS];   // column-band [n_rad][2w+1]: Rcol[j][e] = R_L[j-w+e][j]
+  const cplx* Rall;        // banded path: column-band of every term interleaved [n_rad][T][2w+1]: Rall[j][L][e] = R_L[j-w+e][j]
+  const int* slot;         // [ld] index of the channel's class in its CTA's class list, -1 = not staged
+  const int* cta_cls;      // [n_cta][TDDE_AP_MAXC] classes staged per CTA (-1 = unused)
   const cplx* Aoff;        // banded path: [n_slots][ld], slot = (term, offset) in kernel order
   // generic path
   const int* A_rowptr[TDDE_MAX_TERMS];
