@@ -55,6 +55,7 @@ bool band_lu(std::vector<zc>& M, int n, int w, zc* Lcol, zc* Ucol) {
     for (int d = 1; d <= w; ++d) Lcol[(size_t)i * w + d - 1] = (i + d < n) ? at(i + d, i) : zc(0, 0);
     Ucol[(size_t)i * (w + 1)] = zc(1, 0) / at(i, i);
     for (int d = 1; d <= w; ++d) Ucol[(size_t)i * (w + 1) + d] = (i - d >= 0) ? at(i - d, i) : zc(0, 0);
+    Ucol[(size_t)i * (w + 1) + 1] *= Ucol[(size_t)i * (w + 1)];   // pre-scaled: shortens the dependent chain of the U sweep
   }
   return true;
 }
@@ -119,7 +120,7 @@ bool detect_banded(const tdde_config* c, const tdde_term* terms, int* m0, int* m
 extern "C" void tdde_destroy(tdde_handle* h) {
   if (!h) return;
   cudaStreamSynchronize(h->stream);
-  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_Lcol, h->d_Ucol, h->X, h->r,
+  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_pslot, h->d_warp_cls, h->d_Lcol, h->d_Ucol, h->X, h->r,
                   h->rhat, h->p, h->v, h->s, h->t, h->y, h->z, h->c_stage, h->d_st, h->d_st_bench, h->d_partials,
                   h->d_ticket, h->d_g, h->d_g_small, h->d_zero_g};
   for (void* p : ptrs) if (p) cudaFree(p);
@@ -179,6 +180,25 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     for (int a = 0; a < c.n_ang; ++a) cls[a] = cls_of_chan[a];
     int rc = dev_upload(&h->d_cls, cls.data(), cls.size(), s);
     if (rc) return rc;
+    CU(cudaStreamSynchronize(s));
+  }
+  // preconditioner: per warp (32 consecutive channels) the first TDDE_PC_MAXC distinct classes are staged
+  {
+    const int n_warp = h->ld / 32;
+    std::vector<int> slot(h->ld, -1), wcls((size_t)n_warp * TDDE_PC_MAXC, -1);
+    for (int b = 0; b < n_warp; ++b) {
+      int cnt = 0;
+      for (int a = b * 32; a < (b + 1) * 32; ++a) {
+        const int k = a < c.n_ang ? cls_of_chan[a] : 0;
+        int q = 0;
+        while (q < cnt && wcls[(size_t)b * TDDE_PC_MAXC + q] != k) ++q;
+        if (q == cnt && cnt < TDDE_PC_MAXC) wcls[(size_t)b * TDDE_PC_MAXC + cnt++] = k;
+        slot[a] = q < cnt ? q : -1;
+      }
+    }
+    int rc;
+    if ((rc = dev_upload(&h->d_pslot, slot.data(), slot.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_warp_cls, wcls.data(), wcls.size(), s))) return rc;
     CU(cudaStreamSynchronize(s));
   }
   // block bands S, H0, M+ in the layout of the chosen path; LU of M+

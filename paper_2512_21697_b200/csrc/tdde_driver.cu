@@ -59,7 +59,9 @@ int enqueue_precond(tdde_handle* h, const cplx* x, cplx* y, const SolverState* s
   PrecArgs p;
   p.x = x; p.y = y; p.n_ang = h->cfg.n_ang; p.n_rad = h->cfg.n_rad; p.ld = h->ld; p.w = h->cfg.w0;
   p.cls = h->d_cls; p.Lcol = h->d_Lcol; p.Ucol = h->d_Ucol; p.st = st;
+  p.slot = h->d_pslot; p.warp_cls = h->d_warp_cls;
   int rc = launch_precond(p, h->stream);
+  if (rc == -2) return tdde_cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(precond)");
   if (rc < 0) return TDDE_EINVAL;
   h->launches += rc;
   return 0;

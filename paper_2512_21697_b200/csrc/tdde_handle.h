@@ -34,6 +34,7 @@ struct tdde_handle {
   int* d_Acol[TDDE_MAX_TERMS] = {};
   cplx* d_Aval[TDDE_MAX_TERMS] = {};
   cplx *d_Lcol = nullptr, *d_Ucol = nullptr; // preconditioner factors
+  int *d_pslot = nullptr, *d_warp_cls = nullptr;
 
   // work vectors (internal layout)
   cplx *X = nullptr, *r = nullptr, *rhat = nullptr, *p = nullptr, *v = nullptr, *s = nullptr, *t = nullptr,

@@ -15,6 +15,7 @@
 #define TDDE_TINY 1e-290
 #define TDDE_AP_JC 8
 #define TDDE_AP_MAXC 4
+#define TDDE_PC_MAXC 8
 
 typedef double2 cplx;
 
@@ -102,7 +103,9 @@ struct PrecArgs {
   int n_ang, n_rad, ld, w;
   const int* cls;
   const cplx* Lcol;        // [n_cls][n_rad][w]:  Lcol[k][i][d-1] = L_k[i+d][i]
-  const cplx* Ucol;        // [n_cls][n_rad][w+1]: Ucol[k][i][0] = 1/U_k[i][i], Ucol[k][i][d] = U_k[i-d][i]
+  const cplx* Ucol;        // [n_cls][n_rad][w+1]: [0] = 1/U_k[i][i], [1] = U_k[i-1][i]/U_k[i][i], [d>=2] = U_k[i-d][i]
+  const int* slot;         // [ld] index of the channel's class in its warp's class list, -1 = not staged
+  const int* warp_cls;     // [ld/32][TDDE_PC_MAXC] classes staged per warp (-1 = unused)
   const SolverState* st;   // nullable guard
 };
 

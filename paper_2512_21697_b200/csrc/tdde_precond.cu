@@ -1,107 +1,168 @@
 // tdde_precond.cu -- y = (S + i dt/2 H0)^{-1} x as batched banded triangular solves (
 // PAPER.md:211-215, Eq. 26: M is block-diagonal over angular channels, LU factors computed at start-up).
 //
-// One thread per angular channel, lanes = consecutive channels (coalesced 16-byte accesses in the internal
-// layout).  Both sweeps run in column-oriented (axpy) form: once y_i is final, the W pending rows below it
-// are updated independently, so the dependent chain per row is a single complex FMA and the remaining W-1
-// updates are instruction-level parallel.  Unit-lower L: Lcol[k][i][d-1] = L[i+d][i];  U: Ucol[k][i][0] =
-// 1/U[i][i], Ucol[k][i][d] = U[i-d][i].  Coefficients are per-lane loads indexed by the channel's class;
-// lanes of the same class hit the same address.  Loads for row block n+1 are issued before the dependent
-// chain of block n (software prefetch), because the recurrence itself cannot be parallelised along r.
+// One warp per 32 consecutive angular channels, lane = channel (coalesced 16-byte accesses in the internal
+// layout); the recurrence along r is inherently serial, so the kernel is organised around two facts:
+//  * latency of the dependent chain.  Both sweeps run in column-oriented (axpy) form: once y_i is final the W
+//    pending rows below it are updated independently.  Only the update of the next row is on the critical
+//    path, and it is split as  pw0' = (pw1 - c x_i) - c pw0  so that the chain is one complex FMA (two
+//    dependent DFMAs) per row; for the U sweep the host pre-scales U[i-1][i] by 1/U[i][i] for the same reason.
+//  * few warps (N_ang / 32), so memory latency cannot be hidden by occupancy.  Vector rows and the factor rows
+//    of the (few) kappa-classes present in the warp are streamed through a shared-memory ring with cp.async,
+//    PC_STAGES x PC_ROWS rows ahead of the row being solved.
+// Factor layout (tdde_create.cu): Lcol[k][i][d-1] = L[i+d][i];
+//   Ucol[k][i][0] = 1/U[i][i], Ucol[k][i][1] = U[i-1][i] / U[i][i], Ucol[k][i][d>=2] = U[i-d][i].
 #include "tdde_reduce.cuh"
 
 #define PC_NT 32
-#define PC_UNROLL 4
+#define PC_ROWS 16
+#define PC_STAGES 4
+#define PC_MAXC TDDE_PC_MAXC
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+template <int W>
+struct PrecPlan {
+  static constexpr int CW = W + 1;                                   // coefficient row width (U needs W+1)
+  static constexpr int XS = PC_ROWS * PC_NT;                         // complex per stage
+  static constexpr int CS = PC_MAXC * PC_ROWS * CW;
+  static constexpr int STAGE = XS + CS;
+  static constexpr size_t SMEM = (size_t)PC_STAGES * STAGE * sizeof(cplx);
+};
 
 template <int W>
 __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
+  using PL = PrecPlan<W>;
   if (p.st && solver_idle(p.st)) return;
-  const int a = blockIdx.x * PC_NT + threadIdx.x;
-  if (a >= p.ld) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx* ring = reinterpret_cast<cplx*>(smem_raw);
+  const int lane = threadIdx.x;
+  const int a = blockIdx.x * PC_NT + lane;                           // a < ld always (ld is a multiple of 32)
   const int ld = p.ld, n_rad = p.n_rad;
+  const int* wcls = p.warp_cls + blockIdx.x * PC_MAXC;
+  int ncls = 0;
+#pragma unroll
+  for (int q = 0; q < PC_MAXC; ++q) ncls += (wcls[q] >= 0);
+  const int slot = p.slot[a];
   const int k = p.cls[a];
-  const cplx* Lc = p.Lcol + (size_t)k * n_rad * W;
-  const cplx* Uc = p.Ucol + (size_t)k * n_rad * (W + 1);
+  const int nst = (n_rad + PC_ROWS - 1) / PC_ROWS;
 
   cplx pw[W + 1];
-#pragma unroll
-  for (int d = 0; d <= W; ++d) pw[d] = make_double2(0, 0);
 
-  // ---- forward: L y = x ----
+  // ================= forward: L y = x =================
   {
-    cplx xn[PC_UNROLL], cn[PC_UNROLL][W];
-    auto load = [&](int ib) {
-#pragma unroll
-      for (int u = 0; u < PC_UNROLL; ++u) {
-        const int i = min(ib + u, n_rad - 1);
-        xn[u] = p.x[(size_t)i * ld + a];
-#pragma unroll
-        for (int d = 0; d < W; ++d) cn[u][d] = __ldg(Lc + (size_t)i * W + d);
-      }
-    };
-    load(0);
-    for (int ib = 0; ib < n_rad; ib += PC_UNROLL) {
-      cplx xc[PC_UNROLL], cc[PC_UNROLL][W];
-#pragma unroll
-      for (int u = 0; u < PC_UNROLL; ++u) {
-        xc[u] = xn[u];
-#pragma unroll
-        for (int d = 0; d < W; ++d) cc[u][d] = cn[u][d];
-      }
-      if (ib + PC_UNROLL < n_rad) load(ib + PC_UNROLL);
-#pragma unroll
-      for (int u = 0; u < PC_UNROLL; ++u) {
-        const int i = ib + u;
-        if (i < n_rad) {
-          const cplx yi = cadd(xc[u], pw[0]);
-          p.y[(size_t)i * ld + a] = yi;
-          const cplx nyi = make_double2(-yi.x, -yi.y);
-#pragma unroll
-          for (int d = 0; d < W; ++d) { pw[d] = pw[d + 1]; cfma(pw[d], cc[u][d], nyi); }
+    auto issue = [&](int s) {                                        // rows [s*R, s*R + R)
+      if (s < nst) {
+        cplx* st = ring + (size_t)(s % PC_STAGES) * PL::STAGE;
+        const int r0 = s * PC_ROWS, nr = min(PC_ROWS, n_rad - r0);
+        for (int r = 0; r < nr; ++r) cp_async16(st + r * PC_NT + lane, p.x + (size_t)(r0 + r) * ld + a);
+        for (int q = 0; q < ncls; ++q) {
+          const cplx* src = p.Lcol + ((size_t)wcls[q] * n_rad + r0) * W;
+          cplx* dst = st + PL::XS + (size_t)q * PC_ROWS * PL::CW;
+          for (int e = lane; e < nr * W; e += PC_NT) cp_async16(dst + e, src + e);
         }
       }
+      cp_async_commit();
+    };
+#pragma unroll
+    for (int d = 0; d <= W; ++d) pw[d] = make_double2(0, 0);
+    for (int s = 0; s < PC_STAGES - 1; ++s) issue(s);
+    for (int s = 0; s < nst; ++s) {
+      issue(s + PC_STAGES - 1);
+      cp_async_wait<PC_STAGES - 1>();
+      __syncwarp();
+      const cplx* st = ring + (size_t)(s % PC_STAGES) * PL::STAGE;
+      const int r0 = s * PC_ROWS, nr = min(PC_ROWS, n_rad - r0);
+      const cplx* cs = st + PL::XS + (size_t)(slot >= 0 ? slot : 0) * PC_ROWS * PL::CW;
+      const cplx* cg = p.Lcol + ((size_t)k * n_rad + r0) * W;
+#pragma unroll 4
+      for (int r = 0; r < nr; ++r) {
+        const cplx xi = st[r * PC_NT + lane];
+        cplx c[W];
+        if (slot >= 0) {
+#pragma unroll
+          for (int d = 0; d < W; ++d) c[d] = cs[r * W + d];
+        } else {
+#pragma unroll
+          for (int d = 0; d < W; ++d) c[d] = __ldg(cg + r * W + d);
+        }
+        const cplx nc0 = make_double2(-c[0].x, -c[0].y);
+        cplx base = pw[1];
+        cfma(base, nc0, xi);                                         // off the chain
+        const cplx yi = cadd(xi, pw[0]);
+        p.y[(size_t)(r0 + r) * ld + a] = yi;
+        const cplx nyi = make_double2(-yi.x, -yi.y);
+        cfma(base, nc0, pw[0]);                                      // the chain: one complex FMA per row
+        pw[0] = base;
+#pragma unroll
+        for (int d = 1; d < W; ++d) { pw[d] = pw[d + 1]; cfma(pw[d], c[d], nyi); }
+      }
+      __syncwarp();
     }
+    cp_async_wait<0>();
+    __threadfence();   // the U sweep re-reads, asynchronously, what this thread just stored
   }
-#pragma unroll
-  for (int d = 0; d <= W; ++d) pw[d] = make_double2(0, 0);
-  // ---- backward: U x = y ----
+  // ================= backward: U x = y (rows descending; stage s covers rows [n_rad - (s+1) R, n_rad - s R)) ====
   {
-    cplx xn[PC_UNROLL], cn[PC_UNROLL][W + 1];
-    auto load = [&](int ib) {          // rows ib, ib-1, ...
-#pragma unroll
-      for (int u = 0; u < PC_UNROLL; ++u) {
-        const int i = max(ib - u, 0);
-        xn[u] = p.y[(size_t)i * ld + a];
-#pragma unroll
-        for (int d = 0; d <= W; ++d) cn[u][d] = __ldg(Uc + (size_t)i * (W + 1) + d);
-      }
-    };
-    load(n_rad - 1);
-    for (int ib = n_rad - 1; ib >= 0; ib -= PC_UNROLL) {
-      cplx xc[PC_UNROLL], cc[PC_UNROLL][W + 1];
-#pragma unroll
-      for (int u = 0; u < PC_UNROLL; ++u) {
-        xc[u] = xn[u];
-#pragma unroll
-        for (int d = 0; d <= W; ++d) cc[u][d] = cn[u][d];
-      }
-      if (ib - PC_UNROLL >= 0) load(ib - PC_UNROLL);
-#pragma unroll
-      for (int u = 0; u < PC_UNROLL; ++u) {
-        const int i = ib - u;
-        if (i >= 0) {
-          const cplx xi = cmul(cadd(xc[u], pw[0]), cc[u][0]);
-          p.y[(size_t)i * ld + a] = xi;
-          const cplx nxi = make_double2(-xi.x, -xi.y);
-#pragma unroll
-          for (int d = 0; d < W; ++d) { pw[d] = pw[d + 1]; cfma(pw[d], cc[u][d + 1], nxi); }
+    auto issue = [&](int s) {
+      if (s < nst) {
+        cplx* st = ring + (size_t)(s % PC_STAGES) * PL::STAGE;
+        const int hi = n_rad - s * PC_ROWS, lo = max(0, hi - PC_ROWS), nr = hi - lo;
+        for (int r = 0; r < nr; ++r) cp_async16(st + r * PC_NT + lane, p.y + (size_t)(lo + r) * ld + a);
+        for (int q = 0; q < ncls; ++q) {
+          const cplx* src = p.Ucol + ((size_t)wcls[q] * n_rad + lo) * (W + 1);
+          cplx* dst = st + PL::XS + (size_t)q * PC_ROWS * PL::CW;
+          for (int e = lane; e < nr * (W + 1); e += PC_NT) cp_async16(dst + e, src + e);
         }
       }
+      cp_async_commit();
+    };
+#pragma unroll
+    for (int d = 0; d <= W; ++d) pw[d] = make_double2(0, 0);
+    for (int s = 0; s < PC_STAGES - 1; ++s) issue(s);
+    for (int s = 0; s < nst; ++s) {
+      issue(s + PC_STAGES - 1);
+      cp_async_wait<PC_STAGES - 1>();
+      __syncwarp();
+      const cplx* st = ring + (size_t)(s % PC_STAGES) * PL::STAGE;
+      const int hi = n_rad - s * PC_ROWS, lo = max(0, hi - PC_ROWS), nr = hi - lo;
+      const cplx* cs = st + PL::XS + (size_t)(slot >= 0 ? slot : 0) * PC_ROWS * PL::CW;
+      const cplx* cg = p.Ucol + ((size_t)k * n_rad + lo) * (W + 1);
+#pragma unroll 4
+      for (int r = nr - 1; r >= 0; --r) {
+        const cplx yi = st[r * PC_NT + lane];
+        cplx c[W + 1];
+        if (slot >= 0) {
+#pragma unroll
+          for (int d = 0; d <= W; ++d) c[d] = cs[r * (W + 1) + d];
+        } else {
+#pragma unroll
+          for (int d = 0; d <= W; ++d) c[d] = __ldg(cg + r * (W + 1) + d);
+        }
+        // x_i = uinv (y_i + pw0);  pw0' = pw1 - U[i-1][i] x_i = (pw1 - c1 y_i) - c1 pw0  with c1 = U[i-1][i] uinv
+        const cplx nc1 = make_double2(-c[1].x, -c[1].y);
+        cplx base = pw[1];
+        cfma(base, nc1, yi);                                         // off the chain
+        const cplx xi = cmul(cadd(yi, pw[0]), c[0]);
+        p.y[(size_t)(lo + r) * ld + a] = xi;
+        const cplx nxi = make_double2(-xi.x, -xi.y);
+        cfma(base, nc1, pw[0]);                                      // the chain
+        pw[0] = base;
+#pragma unroll
+        for (int d = 1; d < W; ++d) { pw[d] = pw[d + 1]; cfma(pw[d], c[d + 1], nxi); }
+      }
+      __syncwarp();
     }
+    cp_async_wait<0>();
   }
 }
 
-// runtime-w fallback (w <= 32): pending rows in a small circular local array
+// runtime-w fallback (w <= 32): pending rows in a small local array, direct global loads
 __global__ void __launch_bounds__(PC_NT) k_precond_any(const PrecArgs p) {
   if (p.st && solver_idle(p.st)) return;
   const int a = blockIdx.x * PC_NT + threadIdx.x;
@@ -121,23 +182,37 @@ __global__ void __launch_bounds__(PC_NT) k_precond_any(const PrecArgs p) {
   for (int d = 0; d <= W; ++d) pw[d] = make_double2(0, 0);
   for (int i = n_rad - 1; i >= 0; --i) {
     const cplx* uc = Uc + (size_t)i * (W + 1);
-    const cplx xi = cmul(cadd(p.y[(size_t)i * ld + a], pw[0]), uc[0]);
+    const cplx t = cadd(p.y[(size_t)i * ld + a], pw[0]);
+    const cplx xi = cmul(t, uc[0]);
     p.y[(size_t)i * ld + a] = xi;
     const cplx nxi = make_double2(-xi.x, -xi.y);
-    for (int d = 0; d < W; ++d) { pw[d] = pw[d + 1]; cfma(pw[d], uc[d + 1], nxi); }
+    // Ucol[.][1] is pre-scaled by 1/U[i][i]: it multiplies (y_i + pw0), not x_i
+    if (W >= 1) { pw[0] = pw[1]; cfma(pw[0], uc[1], make_double2(-t.x, -t.y)); }
+    for (int d = 1; d < W; ++d) { pw[d] = pw[d + 1]; cfma(pw[d], uc[d + 1], nxi); }
   }
 }
 
+template <int W>
+static int launch_precond_w(const PrecArgs& a, cudaStream_t s) {
+  static bool attr_set = false;
+  const size_t smem = PrecPlan<W>::SMEM;
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(k_precond<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -2;
+    attr_set = true;
+  }
+  k_precond<W><<<a.ld / PC_NT, PC_NT, smem, s>>>(a);
+  return 1;
+}
+
 int launch_precond(const PrecArgs& a, cudaStream_t s) {
-  const int grid = (a.ld + PC_NT - 1) / PC_NT;
   switch (a.w) {
-    case 3: k_precond<3><<<grid, PC_NT, 0, s>>>(a); break;
-    case 6: k_precond<6><<<grid, PC_NT, 0, s>>>(a); break;
-    case 9: k_precond<9><<<grid, PC_NT, 0, s>>>(a); break;
-    case 13: k_precond<13><<<grid, PC_NT, 0, s>>>(a); break;
+    case 3: return launch_precond_w<3>(a, s);
+    case 6: return launch_precond_w<6>(a, s);
+    case 9: return launch_precond_w<9>(a, s);
+    case 13: return launch_precond_w<13>(a, s);
     default:
       if (a.w > 32 || a.w < 1) return -1;
-      k_precond_any<<<grid, PC_NT, 0, s>>>(a);
+      k_precond_any<<<(a.ld + PC_NT - 1) / PC_NT, PC_NT, 0, s>>>(a);
   }
   return 1;
 }
