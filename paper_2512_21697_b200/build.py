@@ -18,7 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 INCLUDE = os.path.join(ROOT, "include")
 OUT = os.path.join(HERE, "libtdde.so")
-SOURCES = ["tdde_apply.cu", "tdde_vec.cu", "tdde_precond.cu", "tdde_create.cu", "tdde_driver.cu", "tdde_misc.cu"]
+SOURCES = ["tdde_apply.cu", "tdde_vec.cu", "tdde_precond.cu", "tdde_partition.cu", "tdde_create.cu", "tdde_driver.cu", "tdde_misc.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--use_fast_math=false"]
 

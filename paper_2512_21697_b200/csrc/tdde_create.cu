@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 #include "tdde_handle.h"
+#include "tdde_partition.h"
 
 thread_local std::string g_last_cuda_error;
 
@@ -34,30 +35,6 @@ void row_to_col_band(const zc* row, zc* col, int n, int w) {
       const int i = j - w + e;
       col[(size_t)j * nd + e] = (i >= 0 && i < n) ? row[(size_t)i * nd + (2 * w - e)] : zc(0, 0);
     }
-}
-
-// LU without pivoting of one band matrix given as row-band; fills Lcol [n][w], Ucol [n][w+1] (tdde_internal.h).
-// No fill leaves the band.  Returns false on a zero / non-finite pivot.
-bool band_lu(std::vector<zc>& M, int n, int w, zc* Lcol, zc* Ucol) {
-  const int nd = 2 * w + 1;
-  auto at = [&](int i, int j) -> zc& { return M[(size_t)i * nd + (j - i + w)]; };
-  for (int i = 0; i < n; ++i) {
-    const zc piv = at(i, i);
-    if (!(std::isfinite(piv.real()) && std::isfinite(piv.imag())) || std::abs(piv) < TDDE_TINY) return false;
-    const int last = std::min(i + w, n - 1);
-    for (int r = i + 1; r <= last; ++r) {
-      const zc l = at(r, i) / piv;
-      at(r, i) = l;
-      for (int c = i + 1; c <= last; ++c) at(r, c) -= l * at(i, c);
-    }
-  }
-  for (int i = 0; i < n; ++i) {
-    for (int d = 1; d <= w; ++d) Lcol[(size_t)i * w + d - 1] = (i + d < n) ? at(i + d, i) : zc(0, 0);
-    Ucol[(size_t)i * (w + 1)] = zc(1, 0) / at(i, i);
-    for (int d = 1; d <= w; ++d) Ucol[(size_t)i * (w + 1) + d] = (i - d >= 0) ? at(i - d, i) : zc(0, 0);
-    Ucol[(size_t)i * (w + 1) + 1] *= Ucol[(size_t)i * (w + 1)];   // pre-scaled: shortens the dependent chain of the U sweep
-  }
-  return true;
 }
 
 int validate(const tdde_config* c, const tdde_c64* S, const tdde_c64* H0, const int32_t* cls, const tdde_term* terms) {
@@ -120,7 +97,7 @@ bool detect_banded(const tdde_config* c, const tdde_term* terms, int* m0, int* m
 extern "C" void tdde_destroy(tdde_handle* h) {
   if (!h) return;
   cudaStreamSynchronize(h->stream);
-  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_pslot, h->d_warp_cls, h->d_Lcol, h->d_Ucol, h->X, h->r,
+  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_pslot, h->d_warp_cls, h->d_Esp, h->d_Msep, h->d_Scinv, h->d_rs, h->d_Lcol, h->d_Ucol, h->X, h->r,
                   h->rhat, h->p, h->v, h->s, h->t, h->y, h->z, h->c_stage, h->d_st, h->d_st_bench, h->d_partials,
                   h->d_ticket, h->d_g, h->d_g_small, h->d_zero_g};
   for (void* p : ptrs) if (p) cudaFree(p);
@@ -205,6 +182,18 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
   {
     std::vector<zc> Sx(h->blk_count), Hx(h->blk_count), Mx(h->blk_count);
     std::vector<zc> Lc((size_t)c.n_cls * n_rad * w0), Uc((size_t)c.n_cls * n_rad * (w0 + 1));
+    // partition count of the preconditioner solve: about 1.5 warps per SM sub-partition (4 x 148), interiors >= 8 w0
+    int P = (int)((888 + h->ld / 32 - 1) / (h->ld / 32));
+    if (const char* env = std::getenv("TDDE_PC_PARTS")) P = std::atoi(env);
+    const bool templated_w = (w0 == 3 || w0 == 6 || w0 == 9 || w0 == 13);
+    P = templated_w ? std::min(std::max(P, 1), TDDE_PC_MAXPARTS) : 1;
+    const PartitionPlan plan = make_partition_plan(n_rad, w0, P);
+    h->pc_P = plan.P; h->pc_ns = plan.ns();
+    for (int q = 0; q < plan.P; ++q) { h->pc_range_lo[q] = plan.lo[q]; h->pc_int_hi[q] = plan.hi[q]; }
+    for (int q = plan.P; q <= TDDE_PC_MAXPARTS; ++q) h->pc_range_lo[q] = n_rad;
+    const int ns = plan.ns();
+    std::vector<zc> Esp(plan.P > 1 ? (size_t)c.n_cls * n_rad * 2 * w0 : 1), Msep(plan.P > 1 ? (size_t)c.n_cls * ns * nd0 : 1),
+        Scinv(plan.P > 1 ? (size_t)c.n_cls * ns * ns : 1);
     std::vector<zc> Mrow(blk_sz);
     const zc itau(0.0, h->tau);
     for (int k = 0; k < c.n_cls; ++k) {
@@ -224,7 +213,10 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
         std::memcpy(&Hx[k * blk_sz], Hk, blk_sz * sizeof(zc));
         std::memcpy(&Mx[k * blk_sz], Mrow.data(), blk_sz * sizeof(zc));
       }
-      if (!band_lu(Mrow, n_rad, w0, &Lc[(size_t)k * n_rad * w0], &Uc[(size_t)k * n_rad * (w0 + 1)]))
+      if (!build_partitioned_factors(Mrow, plan, &Lc[(size_t)k * n_rad * w0], &Uc[(size_t)k * n_rad * (w0 + 1)],
+                                     plan.P > 1 ? &Esp[(size_t)k * n_rad * 2 * w0] : nullptr,
+                                     plan.P > 1 ? &Msep[(size_t)k * ns * nd0] : nullptr,
+                                     plan.P > 1 ? &Scinv[(size_t)k * ns * ns] : nullptr))
         return TDDE_ESINGULAR;
     }
     int rc;
@@ -234,6 +226,10 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     if ((rc = dev_upload(&h->d_blk_tmp, (cplx*)nullptr, Mx.size(), s))) return rc;
     if ((rc = dev_upload(&h->d_Lcol, reinterpret_cast<cplx*>(Lc.data()), Lc.size(), s))) return rc;
     if ((rc = dev_upload(&h->d_Ucol, reinterpret_cast<cplx*>(Uc.data()), Uc.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_Esp, reinterpret_cast<cplx*>(Esp.data()), Esp.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_Msep, reinterpret_cast<cplx*>(Msep.data()), Msep.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_Scinv, reinterpret_cast<cplx*>(Scinv.data()), Scinv.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_rs, (cplx*)nullptr, (size_t)std::max(ns, 1) * h->ld, s))) return rc;
     CU(cudaStreamSynchronize(s));
   }
   // coupling terms

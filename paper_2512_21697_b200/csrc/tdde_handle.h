@@ -35,6 +35,9 @@ struct tdde_handle {
   cplx* d_Aval[TDDE_MAX_TERMS] = {};
   cplx *d_Lcol = nullptr, *d_Ucol = nullptr; // preconditioner factors
   int *d_pslot = nullptr, *d_warp_cls = nullptr;
+  int pc_P = 1, pc_ns = 0;                   // partitioned solve (tdde_partition.h)
+  int pc_range_lo[TDDE_PC_MAXPARTS + 1] = {}, pc_int_hi[TDDE_PC_MAXPARTS] = {};
+  cplx *d_Esp = nullptr, *d_Msep = nullptr, *d_Scinv = nullptr, *d_rs = nullptr;
 
   // work vectors (internal layout)
   cplx *X = nullptr, *r = nullptr, *rhat = nullptr, *p = nullptr, *v = nullptr, *s = nullptr, *t = nullptr,

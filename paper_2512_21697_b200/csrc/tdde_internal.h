@@ -16,6 +16,7 @@
 #define TDDE_AP_JC 8
 #define TDDE_AP_MAXC 4
 #define TDDE_PC_MAXC 8
+#define TDDE_PC_MAXPARTS 16
 
 typedef double2 cplx;
 
@@ -106,6 +107,14 @@ struct PrecArgs {
   const cplx* Ucol;        // [n_cls][n_rad][w+1]: [0] = 1/U_k[i][i], [1] = U_k[i-1][i]/U_k[i][i], [d>=2] = U_k[i-d][i]
   const int* slot;         // [ld] index of the channel's class in its warp's class list, -1 = not staged
   const int* warp_cls;     // [ld/32][TDDE_PC_MAXC] classes staged per warp (-1 = unused)
+  // partitioned solve (tdde_partition.h); P == 1: plain LU over all rows
+  int P, ns;
+  int range_lo[TDDE_PC_MAXPARTS + 1];   // range q = rows [range_lo[q], range_lo[q+1]) = interior q + separator after it
+  int int_hi[TDDE_PC_MAXPARTS];         // interior q = rows [range_lo[q], int_hi[q])
+  const cplx* Esp;         // [n_cls][n_rad][2w]
+  const cplx* Msep;        // [n_cls][ns][2w+1]
+  const cplx* Scinv;       // [n_cls][ns][ns]
+  cplx* rs;                // scratch [ns][ld]: Schur right-hand side
   const SolverState* st;   // nullable guard
 };
 

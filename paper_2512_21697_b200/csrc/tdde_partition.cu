@@ -1,0 +1,148 @@
+// tdde_partition.cu -- host code (one-time, per kappa-class): see tdde_partition.h.
+#include <algorithm>
+#include <cmath>
+#include "tdde_internal.h"
+#include "tdde_partition.h"
+
+PartitionPlan make_partition_plan(int n, int w, int P) {
+  PartitionPlan pl;
+  pl.n = n; pl.w = w;
+  P = std::max(1, P);
+  while (P > 1 && (n - (P - 1) * w) / P < 8 * w) --P;     // interiors must dominate the separators
+  pl.P = P;
+  const int interior = n - (P - 1) * w;
+  int pos = 0;
+  for (int q = 0; q < P; ++q) {
+    const int m = interior / P + (q < interior % P ? 1 : 0);
+    pl.lo.push_back(pos);
+    pl.hi.push_back(pos + m);
+    pos += m + w;
+  }
+  return pl;
+}
+
+namespace {
+
+// segment id of a row: 2q for interior q, 2q+1 for the separator after interior q
+int segment_of(const PartitionPlan& pl, int i) {
+  for (int q = 0; q < pl.P; ++q) {
+    if (i < pl.hi[q]) return 2 * q;
+    if (q + 1 < pl.P && i < pl.lo[q + 1]) return 2 * q + 1;
+  }
+  return 2 * (pl.P - 1);
+}
+
+bool invert_dense(std::vector<zc>& A, int n, zc* out) {   // Gauss-Jordan, partial pivoting
+  std::vector<zc> I((size_t)n * n, zc(0, 0));
+  for (int i = 0; i < n; ++i) I[(size_t)i * n + i] = zc(1, 0);
+  for (int c = 0; c < n; ++c) {
+    int piv = c;
+    double best = std::abs(A[(size_t)c * n + c]);
+    for (int r = c + 1; r < n; ++r)
+      if (std::abs(A[(size_t)r * n + c]) > best) { best = std::abs(A[(size_t)r * n + c]); piv = r; }
+    if (!(best > TDDE_TINY) || !std::isfinite(best)) return false;
+    if (piv != c)
+      for (int j = 0; j < n; ++j) { std::swap(A[(size_t)c * n + j], A[(size_t)piv * n + j]); std::swap(I[(size_t)c * n + j], I[(size_t)piv * n + j]); }
+    const zc inv = zc(1, 0) / A[(size_t)c * n + c];
+    for (int j = 0; j < n; ++j) { A[(size_t)c * n + j] *= inv; I[(size_t)c * n + j] *= inv; }
+    for (int r = 0; r < n; ++r) {
+      if (r == c) continue;
+      const zc f = A[(size_t)r * n + c];
+      if (f == zc(0, 0)) continue;
+      for (int j = 0; j < n; ++j) { A[(size_t)r * n + j] -= f * A[(size_t)c * n + j]; I[(size_t)r * n + j] -= f * I[(size_t)c * n + j]; }
+    }
+  }
+  std::copy(I.begin(), I.end(), out);
+  return true;
+}
+
+}  // namespace
+
+bool build_partitioned_factors(const std::vector<zc>& Mrow, const PartitionPlan& pl, zc* Lcol, zc* Ucol, zc* Esp,
+                               zc* Msep, zc* Scinv) {
+  const int n = pl.n, w = pl.w, nd = 2 * w + 1, P = pl.P, ns = pl.ns();
+  auto M = [&](int i, int j) -> zc { return (j < 0 || j >= n || std::abs(i - j) > w) ? zc(0, 0) : Mrow[(size_t)i * nd + (j - i + w)]; };
+  std::vector<int> seg(n);
+  for (int i = 0; i < n; ++i) seg[i] = segment_of(pl, i);
+
+  // block-diagonal copy: couplings between different segments removed, separators replaced by identity
+  std::vector<zc> F(Mrow);
+  for (int i = 0; i < n; ++i)
+    for (int d = -w; d <= w; ++d) {
+      const int j = i + d;
+      if (j < 0 || j >= n) { F[(size_t)i * nd + d + w] = zc(0, 0); continue; }
+      if (seg[i] % 2 == 1) F[(size_t)i * nd + d + w] = (d == 0) ? zc(1, 0) : zc(0, 0);
+      else if (seg[j] != seg[i]) F[(size_t)i * nd + d + w] = zc(0, 0);
+    }
+  auto at = [&](int i, int j) -> zc& { return F[(size_t)i * nd + (j - i + w)]; };
+  // LU without pivoting, in place (block-diagonal structure is preserved: no fill across zeroed couplings)
+  for (int i = 0; i < n; ++i) {
+    const zc piv = at(i, i);
+    if (!(std::isfinite(piv.real()) && std::isfinite(piv.imag())) || std::abs(piv) < TDDE_TINY) return false;
+    const int last = std::min(i + w, n - 1);
+    for (int r = i + 1; r <= last; ++r) {
+      if (at(r, i) == zc(0, 0)) continue;
+      const zc l = at(r, i) / piv;
+      at(r, i) = l;
+      for (int c = i + 1; c <= last; ++c) at(r, c) -= l * at(i, c);
+    }
+  }
+  for (int i = 0; i < n; ++i) {
+    for (int d = 1; d <= w; ++d) Lcol[(size_t)i * w + d - 1] = (i + d < n) ? at(i + d, i) : zc(0, 0);
+    const zc uinv = zc(1, 0) / at(i, i);
+    Ucol[(size_t)i * (w + 1)] = uinv;
+    for (int d = 1; d <= w; ++d) Ucol[(size_t)i * (w + 1) + d] = (i - d >= 0) ? at(i - d, i) : zc(0, 0);
+    Ucol[(size_t)i * (w + 1) + 1] *= uinv;     // pre-scaled: shortens the dependent chain of the U sweep
+  }
+  if (P == 1) return true;
+
+  // solve with the block LU (host): v <- A_qq^{-1} v on rows [lo, hi)
+  auto block_solve = [&](int lo, int hi, std::vector<zc>& v) {
+    for (int i = lo; i < hi; ++i)
+      for (int d = 1; d <= w && i - d >= lo; ++d) v[i] -= at(i, i - d) * v[i - d];
+    for (int i = hi - 1; i >= lo; --i) {
+      for (int d = 1; d <= w && i + d < hi; ++d) v[i] -= at(i, i + d) * v[i + d];
+      v[i] /= at(i, i);
+    }
+  };
+  // spikes E^- (separator before the interior) and E^+ (separator after)
+  std::fill(Esp, Esp + (size_t)n * 2 * w, zc(0, 0));
+  std::vector<zc> v(n);
+  for (int q = 0; q < P; ++q) {
+    const int lo = pl.lo[q], hi = pl.hi[q];
+    for (int side = 0; side < 2; ++side) {
+      if ((side == 0 && q == 0) || (side == 1 && q == P - 1)) continue;
+      const int s0 = side == 0 ? pl.hi[q - 1] : pl.hi[q];
+      for (int c = 0; c < w; ++c) {
+        for (int i = lo; i < hi; ++i) v[i] = M(i, s0 + c);
+        block_solve(lo, hi, v);
+        for (int i = lo; i < hi; ++i) Esp[(size_t)i * 2 * w + side * w + c] = v[i];
+      }
+    }
+  }
+  // separator rows of M (own-separator columns zeroed) and the Schur complement
+  std::vector<zc> Sc((size_t)ns * ns, zc(0, 0));
+  for (int j = 0; j + 1 < P; ++j) {
+    const int s0 = pl.hi[j];
+    for (int c = 0; c < w; ++c) {
+      const int i = s0 + c, row = j * w + c;
+      for (int d = -w; d <= w; ++d) {
+        const int col = i + d;
+        const bool own = col >= s0 && col < s0 + w;
+        Msep[(size_t)row * nd + d + w] = own ? zc(0, 0) : M(i, col);
+        if (own) Sc[(size_t)row * ns + j * w + (col - s0)] += M(i, col);
+        else if (col >= 0 && col < n) {
+          // interior row `col` of interior q: subtract M(i, col) * E[col][.]
+          const int q = seg[col] / 2;
+          for (int side = 0; side < 2; ++side) {
+            const int jsep = side == 0 ? q - 1 : q;          // separator index of E^-/E^+
+            if (jsep < 0 || jsep >= P - 1) continue;
+            for (int c2 = 0; c2 < w; ++c2)
+              Sc[(size_t)row * ns + jsep * w + c2] -= M(i, col) * Esp[(size_t)col * 2 * w + side * w + c2];
+          }
+        }
+      }
+    }
+  }
+  return invert_dense(Sc, ns, Scinv);
+}

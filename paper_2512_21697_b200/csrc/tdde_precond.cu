@@ -15,8 +15,8 @@
 #include "tdde_reduce.cuh"
 
 #define PC_NT 32
-#define PC_ROWS 16
-#define PC_STAGES 4
+#define PC_ROWS 8
+#define PC_STAGES 3
 #define PC_MAXC TDDE_PC_MAXC
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
@@ -43,7 +43,12 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
   cplx* ring = reinterpret_cast<cplx*>(smem_raw);
   const int lane = threadIdx.x;
   const int a = blockIdx.x * PC_NT + lane;                           // a < ld always (ld is a multiple of 32)
-  const int ld = p.ld, n_rad = p.n_rad;
+  const int ld = p.ld, n_tot = p.n_rad;
+  // rows [row0, row0 + n_rad): interior blockIdx.y plus the separator after it (identity rows in the factors)
+  const int row0 = p.range_lo[blockIdx.y];
+  const int n_rad = p.range_lo[blockIdx.y + 1] - row0;
+  const cplx* xin = p.x + (size_t)row0 * ld;
+  cplx* yout = p.y + (size_t)row0 * ld;
   const int* wcls = p.warp_cls + blockIdx.x * PC_MAXC;
   int ncls = 0;
 #pragma unroll
@@ -60,9 +65,9 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
       if (s < nst) {
         cplx* st = ring + (size_t)(s % PC_STAGES) * PL::STAGE;
         const int r0 = s * PC_ROWS, nr = min(PC_ROWS, n_rad - r0);
-        for (int r = 0; r < nr; ++r) cp_async16(st + r * PC_NT + lane, p.x + (size_t)(r0 + r) * ld + a);
+        for (int r = 0; r < nr; ++r) cp_async16(st + r * PC_NT + lane, xin + (size_t)(r0 + r) * ld + a);
         for (int q = 0; q < ncls; ++q) {
-          const cplx* src = p.Lcol + ((size_t)wcls[q] * n_rad + r0) * W;
+          const cplx* src = p.Lcol + ((size_t)wcls[q] * n_tot + row0 + r0) * W;
           cplx* dst = st + PL::XS + (size_t)q * PC_ROWS * PL::CW;
           for (int e = lane; e < nr * W; e += PC_NT) cp_async16(dst + e, src + e);
         }
@@ -79,7 +84,7 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
       const cplx* st = ring + (size_t)(s % PC_STAGES) * PL::STAGE;
       const int r0 = s * PC_ROWS, nr = min(PC_ROWS, n_rad - r0);
       const cplx* cs = st + PL::XS + (size_t)(slot >= 0 ? slot : 0) * PC_ROWS * PL::CW;
-      const cplx* cg = p.Lcol + ((size_t)k * n_rad + r0) * W;
+      const cplx* cg = p.Lcol + ((size_t)k * n_tot + row0 + r0) * W;
 #pragma unroll 4
       for (int r = 0; r < nr; ++r) {
         const cplx xi = st[r * PC_NT + lane];
@@ -95,7 +100,7 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
         cplx base = pw[1];
         cfma(base, nc0, xi);                                         // off the chain
         const cplx yi = cadd(xi, pw[0]);
-        p.y[(size_t)(r0 + r) * ld + a] = yi;
+        yout[(size_t)(r0 + r) * ld + a] = yi;
         const cplx nyi = make_double2(-yi.x, -yi.y);
         cfma(base, nc0, pw[0]);                                      // the chain: one complex FMA per row
         pw[0] = base;
@@ -113,9 +118,9 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
       if (s < nst) {
         cplx* st = ring + (size_t)(s % PC_STAGES) * PL::STAGE;
         const int hi = n_rad - s * PC_ROWS, lo = max(0, hi - PC_ROWS), nr = hi - lo;
-        for (int r = 0; r < nr; ++r) cp_async16(st + r * PC_NT + lane, p.y + (size_t)(lo + r) * ld + a);
+        for (int r = 0; r < nr; ++r) cp_async16(st + r * PC_NT + lane, yout + (size_t)(lo + r) * ld + a);
         for (int q = 0; q < ncls; ++q) {
-          const cplx* src = p.Ucol + ((size_t)wcls[q] * n_rad + lo) * (W + 1);
+          const cplx* src = p.Ucol + ((size_t)wcls[q] * n_tot + row0 + lo) * (W + 1);
           cplx* dst = st + PL::XS + (size_t)q * PC_ROWS * PL::CW;
           for (int e = lane; e < nr * (W + 1); e += PC_NT) cp_async16(dst + e, src + e);
         }
@@ -132,7 +137,7 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
       const cplx* st = ring + (size_t)(s % PC_STAGES) * PL::STAGE;
       const int hi = n_rad - s * PC_ROWS, lo = max(0, hi - PC_ROWS), nr = hi - lo;
       const cplx* cs = st + PL::XS + (size_t)(slot >= 0 ? slot : 0) * PC_ROWS * PL::CW;
-      const cplx* cg = p.Ucol + ((size_t)k * n_rad + lo) * (W + 1);
+      const cplx* cg = p.Ucol + ((size_t)k * n_tot + row0 + lo) * (W + 1);
 #pragma unroll 4
       for (int r = nr - 1; r >= 0; --r) {
         const cplx yi = st[r * PC_NT + lane];
@@ -149,7 +154,7 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
         cplx base = pw[1];
         cfma(base, nc1, yi);                                         // off the chain
         const cplx xi = cmul(cadd(yi, pw[0]), c[0]);
-        p.y[(size_t)(lo + r) * ld + a] = xi;
+        yout[(size_t)(lo + r) * ld + a] = xi;
         const cplx nxi = make_double2(-xi.x, -xi.y);
         cfma(base, nc1, pw[0]);                                      // the chain
         pw[0] = base;
@@ -159,6 +164,80 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
       __syncwarp();
     }
     cp_async_wait<0>();
+  }
+}
+
+// ---- kernel B: Schur-complement solve for the separator unknowns (tdde_partition.h), two fully parallel steps ----
+// B1: r_S = b_S - A_SI t_I from the separator rows of M: one thread per (separator row, channel).
+template <int W>
+__global__ void __launch_bounds__(128) k_precond_schur_rhs(const PrecArgs p) {
+  if (p.st && solver_idle(p.st)) return;
+  const int a = blockIdx.x * 128 + threadIdx.x;
+  if (a >= p.ld) return;
+  constexpr int ND = 2 * W + 1;
+  const int srow = blockIdx.y, ld = p.ld, n_rad = p.n_rad;
+  const int i = p.int_hi[srow / W] + srow % W;
+  const cplx* ms = p.Msep + ((size_t)p.cls[a] * p.ns + srow) * ND;
+  cplx acc = p.y[(size_t)i * ld + a];
+#pragma unroll
+  for (int d = -W; d <= W; ++d) {
+    const int ii = i + d;
+    if (ii >= 0 && ii < n_rad) {
+      const cplx m = __ldg(ms + d + W);
+      cfma(acc, make_double2(-m.x, -m.y), p.y[(size_t)ii * ld + a]);
+    }
+  }
+  p.rs[(size_t)srow * ld + a] = acc;
+}
+// B2: x_S = Sc^{-1} r_S (dense (P-1) w square per class): one thread per (separator row, channel).
+template <int W>
+__global__ void __launch_bounds__(128) k_precond_schur_mul(const PrecArgs p) {
+  if (p.st && solver_idle(p.st)) return;
+  const int a = blockIdx.x * 128 + threadIdx.x;
+  if (a >= p.ld) return;
+  const int o = blockIdx.y, ld = p.ld, ns = p.ns;
+  const cplx* sc = p.Scinv + ((size_t)p.cls[a] * ns + o) * ns;
+  cplx acc[4];
+#pragma unroll
+  for (int u = 0; u < 4; ++u) acc[u] = make_double2(0, 0);
+  int q = 0;
+  for (; q + 3 < ns; q += 4) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) cfma(acc[u], __ldg(sc + q + u), p.rs[(size_t)(q + u) * ld + a]);
+  }
+  for (; q < ns; ++q) cfma(acc[0], __ldg(sc + q), p.rs[(size_t)q * ld + a]);
+  const int row = p.int_hi[o / W] + o % W;
+  p.y[(size_t)row * ld + a] = cadd(cadd(acc[0], acc[1]), cadd(acc[2], acc[3]));
+}
+
+// ---- kernel C: x_I = t_I - E^- x_S(before) - E^+ x_S(after): streaming, 2 W complex FMAs per row ----
+#define PCC_ROWS 64
+template <int W>
+__global__ void __launch_bounds__(128) k_precond_correct(const PrecArgs p) {
+  if (p.st && solver_idle(p.st)) return;
+  const int a = blockIdx.x * 128 + threadIdx.x;
+  if (a >= p.ld) return;
+  const int q = blockIdx.y, ld = p.ld;
+  const int lo = p.range_lo[q], hi = p.int_hi[q];
+  const int i0 = lo + blockIdx.z * PCC_ROWS, i1 = min(hi, i0 + PCC_ROWS);
+  if (i0 >= hi) return;
+  const int k = p.cls[a];
+  cplx xm[W], xp[W];
+#pragma unroll
+  for (int c = 0; c < W; ++c) {
+    xm[c] = q > 0 ? p.y[(size_t)(p.int_hi[q - 1] + c) * ld + a] : make_double2(0, 0);
+    xp[c] = q + 1 < p.P ? p.y[(size_t)(hi + c) * ld + a] : make_double2(0, 0);
+    xm[c] = make_double2(-xm[c].x, -xm[c].y);
+    xp[c] = make_double2(-xp[c].x, -xp[c].y);
+  }
+  const cplx* E = p.Esp + (size_t)k * p.n_rad * 2 * W;
+#pragma unroll 2
+  for (int i = i0; i < i1; ++i) {
+    cplx t = p.y[(size_t)i * ld + a];
+    const cplx* e = E + (size_t)i * 2 * W;
+#pragma unroll
+    for (int c = 0; c < W; ++c) { cfma(t, __ldg(e + c), xm[c]); cfma(t, __ldg(e + W + c), xp[c]); }
+    p.y[(size_t)i * ld + a] = t;
   }
 }
 
@@ -200,8 +279,14 @@ static int launch_precond_w(const PrecArgs& a, cudaStream_t s) {
     if (cudaFuncSetAttribute(k_precond<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -2;
     attr_set = true;
   }
-  k_precond<W><<<a.ld / PC_NT, PC_NT, smem, s>>>(a);
-  return 1;
+  k_precond<W><<<dim3(a.ld / PC_NT, a.P), PC_NT, smem, s>>>(a);
+  if (a.P == 1) return 1;
+  k_precond_schur_rhs<W><<<dim3((a.ld + 127) / 128, a.ns), 128, 0, s>>>(a);
+  k_precond_schur_mul<W><<<dim3((a.ld + 127) / 128, a.ns), 128, 0, s>>>(a);
+  int max_int = 0;
+  for (int q = 0; q < a.P; ++q) max_int = max_int > a.int_hi[q] - a.range_lo[q] ? max_int : a.int_hi[q] - a.range_lo[q];
+  k_precond_correct<W><<<dim3((a.ld + 127) / 128, a.P, (max_int + PCC_ROWS - 1) / PCC_ROWS), 128, 0, s>>>(a);
+  return 4;
 }
 
 int launch_precond(const PrecArgs& a, cudaStream_t s) {
@@ -211,7 +296,7 @@ int launch_precond(const PrecArgs& a, cudaStream_t s) {
     case 9: return launch_precond_w<9>(a, s);
     case 13: return launch_precond_w<13>(a, s);
     default:
-      if (a.w > 32 || a.w < 1) return -1;
+      if (a.w > 32 || a.w < 1 || a.P != 1) return -1;
       k_precond_any<<<(a.ld + PC_NT - 1) / PC_NT, PC_NT, 0, s>>>(a);
   }
   return 1;
