@@ -14,7 +14,7 @@ from typing import Optional
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libtdde.so")
+LIB_PATH = os.environ.get("TDDE_LIB_PATH", os.path.join(_HERE, "libtdde.so"))
 
 EXPORTS = [
     "tdde_create", "tdde_step", "tdde_propagate", "tdde_norm", "tdde_apply", "tdde_precond",

@@ -17,7 +17,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 INCLUDE = os.path.join(ROOT, "include")
-OUT = os.path.join(HERE, "libtdde.so")
+OUT = os.environ.get("TDDE_LIB_OUT", os.path.join(HERE, "libtdde.so"))      # overrides: build-variant experiments
+EXTRA = os.environ.get("TDDE_NVCC_FLAGS", "").split()
 SOURCES = ["tdde_apply.cu", "tdde_vec.cu", "tdde_precond.cu", "tdde_partition.cu", "tdde_create.cu", "tdde_driver.cu", "tdde_misc.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--use_fast_math=false"]
@@ -41,7 +42,7 @@ def _newest_header() -> float:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = _nvcc()
-    bdir = os.path.join(CSRC, "build")
+    bdir = os.path.join(CSRC, "build" + ("_" + "".join(c for c in "".join(EXTRA) if c.isalnum()) if EXTRA else ""))
     os.makedirs(bdir, exist_ok=True)
     hdr_t = _newest_header()
     flags = [f for f in FLAGS if f != "--use_fast_math=false"]
@@ -52,7 +53,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         op = os.path.join(bdir, src.replace(".cu", ".o"))
         objs.append(op)
         if force or not os.path.exists(op) or os.path.getmtime(op) < max(os.path.getmtime(sp), hdr_t):
-            jobs.append((src, [nvcc, *ARCH, *flags, "-I", INCLUDE, "-I", CSRC, "-c", sp, "-o", op]))
+            jobs.append((src, [nvcc, *ARCH, *flags, *EXTRA, "-I", INCLUDE, "-I", CSRC, "-c", sp, "-o", op]))
 
     def run(job):
         name, cmd = job

@@ -16,7 +16,9 @@
 // This kernel is FP64-FMA bound (27-52 flop per HBM byte), not HBM bound.
 #include "tdde_reduce.cuh"
 
-#define AP_NT 128
+#define AP_NT 128            // generic kernel: threads per block
+#define AP_MINB TDDE_AP_MINB
+#define AP_NC TDDE_AP_NC      // banded kernel: channels per CTA
 #define AP_JC TDDE_AP_JC      // radial rows per pipeline stage
 #define AP_MAXC TDDE_AP_MAXC  // distinct kappa-classes per CTA staged in shared memory
 
@@ -59,64 +61,213 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 //   Rs[JC][T][ND]     radial column coefficients of every term (one bulk copy: host stores them [n_rad][T][ND])
 //   Bs[MAXC][JC][ND]  block column coefficients of the (at most MAXC) distinct kappa-classes of this CTA
 //   Xs[JC][XW]        x rows of the CTA's 128 channels plus MAXM halo channels on each side (one bulk copy per row)
-template <int T, int M0, int MS, int W>
+// plus Ps[2][JC][128]: partial outputs handed from warp group 1 to warp group 0 (double-buffered).
+template <int T, int M0, int MS, int W, int NG>
 struct ApplyPlan {
   using SH = BandShape<T, M0, MS>;
   static constexpr int ND = 2 * W + 1;
   static constexpr int MAXM = SH::maxm();
-  static constexpr int XW = AP_NT + 2 * MAXM;
+  static constexpr int XW = AP_NC + 2 * MAXM;
   static constexpr int RS = AP_JC * T * ND;                 // complex elements
   static constexpr int BS = AP_MAXC * AP_JC * ND;
   static constexpr int XS = AP_JC * XW;
   static constexpr int STAGE = RS + BS + XS;
-  static constexpr size_t SMEM = (size_t)2 * STAGE * sizeof(cplx) + 64;
+  static constexpr int PS = (T > 0 && NG == 2) ? 2 * AP_JC * AP_NC : 0;
+  static constexpr int NSTAGE = 3;
+  static constexpr size_t SMEM = (size_t)(NSTAGE * STAGE + PS) * sizeof(cplx) + 64;
+  // Term split: the terms of one channel are shared between two warp groups so that each thread keeps only about
+  // half of the A_L registers (4 warps per SM sub-partition instead of 2).  Group 0 also owns the block part, the
+  // write-out and the fused inner products.  Greedy balance of complex FMAs per row, largest term first.
+  __host__ __device__ static constexpr int cost(int L) { return ND + 2 * SH::m(L); }
+  __host__ __device__ static constexpr int mask() {          // bit L set: term L belongs to group 1
+    int c0 = ND + 4, c1 = 0, mk = 0;
+    for (int L = T - 1; L >= 0; --L) {
+      if (c1 < c0) { c1 += cost(L); mk |= 1 << L; } else c0 += cost(L);
+    }
+    return mk;
+  }
+  __host__ __device__ static constexpr bool mine(int G, int L) { return NG == 1 || ((mask() >> L) & 1) == G; }
+  __host__ __device__ static constexpr int gmaxm(int G) {    // largest channel offset the group touches
+    int m = 0;
+    for (int L = 0; L < T; ++L) if (mine(G, L) && SH::m(L) > m) m = SH::m(L);
+    return m;
+  }
 };
 
-template <int T, int M0, int MS, int W>
-__global__ void __launch_bounds__(AP_NT, 2) k_apply_banded(const ApplyArgs p) {
+struct ApplyCommon {
+  int tid, a, ac, ld, n_rad, i0, i1, jlo, jhi, jend, nchunks, slot;
+  bool lane_ok;
+  cplx* stage_base;
+  cplx* Ps;
+  uint64_t* full;
+  const cplx* blk_g;
+};
+
+// Work of one warp group G over the whole radial segment (see k_apply_banded).
+template <int T, int M0, int MS, int W, int NG, int G, class IssueFn>
+__device__ __forceinline__ void apply_group(const ApplyArgs& p, const ApplyCommon& k, IssueFn issue, cplx& d0, double& d1) {
   using SH = BandShape<T, M0, MS>;
-  using PL = ApplyPlan<T, M0, MS, W>;
-  constexpr int ND = PL::ND, MAXM = PL::MAXM, NS = SH::nslots(), XW = PL::XW, JC = AP_JC;
+  using PL = ApplyPlan<T, M0, MS, W, NG>;
+  constexpr int ND = PL::ND, MAXM = PL::MAXM, NS = SH::nslots(), XW = PL::XW, JC = AP_JC, GM = PL::gmaxm(G);
+  constexpr bool SPLIT = (NG == 2) && (T > 0);
+  constexpr int RU = TDDE_AP_RU;                             // rows unrolled together (register pressure vs ILP)
+  const int ld = k.ld;
+
+  // angular coefficients of this group's terms in registers, pre-multiplied by beta * g_L
+  cplx Areg[NS > 0 ? NS : 1];
+  if (T > 0) {
+    const double* g = p.g + (p.step_ptr ? (size_t)(*p.step_ptr) * T : 0);
+#pragma unroll
+    for (int L = 0; L < T; ++L) {
+      if (!PL::mine(G, L)) continue;
+      const double gl = g[L];
+      const cplx coef = make_double2(p.beta.x * gl, p.beta.y * gl);
+#pragma unroll
+      for (int q = 0; q < 2 * SH::m(L); ++q) {
+        const int s = SH::slot0(L) + q;
+        Areg[s] = cmul(coef, p.Aoff[(size_t)s * ld + k.ac]);
+      }
+    }
+  }
+  cplx yw[ND];
+#pragma unroll
+  for (int e = 0; e < ND; ++e) yw[e] = make_double2(0, 0);
+
+  // Time is cut into slots separated by one CTA barrier.  In slot s group 1 works on chunk s and group 0 on chunk
+  // s - 1, so group 0 finds group 1's partial rows of its chunk already published and can finish every output row
+  // (sum, store, fused inner products) the moment its own part is complete.
+  for (int s = 0; s < k.nchunks + (NG - 1); ++s) {
+    const int c = (G == 1 || NG == 1) ? s : s - 1;
+    if (c >= 0 && c < k.nchunks) {
+      const cplx* st = k.stage_base + (size_t)(c % PL::NSTAGE) * PL::STAGE;
+      cplx* ps = k.Ps + (size_t)(c & 1) * JC * AP_NC;
+      const int jc0 = k.jlo + c * JC;
+      const int nr_real = min(JC, k.jhi - jc0);               // rows with data; later rows of the chunk are virtual
+      const int nr_all = min(JC, k.jend - jc0);
+      if (nr_real > 0) mbar_wait(&k.full[c % PL::NSTAGE], (c / PL::NSTAGE) & 1);
+#pragma unroll RU
+      for (int r = 0; r < nr_all; ++r) {
+        const int i = jc0 + r - W;                            // the output row completed by input row jc0 + r
+        const bool emit = (G == 0) && (i >= k.i0) && k.lane_ok;
+        cplx ax = make_double2(0, 0), pg = make_double2(0, 0);
+        if (G == 0) {
+          if (emit && p.aux) ax = p.aux[(size_t)i * ld + k.a];
+          if (SPLIT) pg = ps[r * AP_NC + k.tid];
+        }
+        if (r < nr_real) {
+          const cplx* xs = st + PL::RS + PL::BS + (size_t)r * XW + k.tid + MAXM;
+          if (G == 0) {
+            const cplx x0 = xs[0];
+            if (k.slot >= 0) {
+              const cplx* bc = st + PL::RS + ((size_t)k.slot * JC + r) * ND;
+#pragma unroll
+              for (int e = 0; e < ND; ++e) cfma(yw[e], bc[e], x0);
+            } else {
+              const cplx* bc = k.blk_g + (size_t)(jc0 + r) * ND;
+#pragma unroll
+              for (int e = 0; e < ND; ++e) cfma(yw[e], __ldg(bc + e), x0);
+            }
+          }
+          if (T > 0 && GM > 0) {
+            cplx z[T > 0 ? T : 1];
+#pragma unroll
+            for (int L = 0; L < T; ++L) z[L] = make_double2(0, 0);
+#pragma unroll
+            for (int o = -GM; o <= GM; ++o) {
+              if (o == 0) continue;
+              const cplx xo = xs[o];
+#pragma unroll
+              for (int L = 0; L < T; ++L) {
+                if (PL::mine(G, L) && SH::m(L) >= (o < 0 ? -o : o)) {
+                  // slot order within a term: o = -m..-1 -> q = o + m ; o = 1..m -> q = m + o - 1
+                  const int q = o < 0 ? o + SH::m(L) : SH::m(L) + o - 1;
+                  cfma(z[L], Areg[SH::slot0(L) + q], xo);
+                }
+              }
+            }
+#pragma unroll
+            for (int L = 0; L < T; ++L) {
+              if (!PL::mine(G, L)) continue;
+              const cplx* rc = st + ((size_t)r * T + L) * ND;  // warp-uniform: broadcast LDS.128
+#pragma unroll
+              for (int e = 0; e < ND; ++e) cfma(yw[e], rc[e], z[L]);
+            }
+          }
+        }
+        if (G == 1) {
+          if (SPLIT) ps[r * AP_NC + k.tid] = yw[0];
+        } else if (emit) {
+          const cplx yv = cadd(yw[0], pg);
+          p.y[(size_t)i * ld + k.a] = yv;
+          cfma_conj(d0, ax, yv);
+          d1 = fma(yv.x, yv.x, d1); d1 = fma(yv.y, yv.y, d1);
+        }
+#pragma unroll
+        for (int e = 0; e < ND - 1; ++e) yw[e] = yw[e + 1];
+        yw[ND - 1] = make_double2(0, 0);
+      }
+    }
+    // both groups are done with their chunks of this slot; group 1's partial rows are published
+    asm volatile("bar.sync 1, %0;" ::"n"(NG * AP_NC) : "memory");
+    if (G == 0 && k.tid == 0 && s + 2 < k.nchunks) issue(s + 2);
+  }
+}
+
+template <int T, int M0, int MS, int W, int NG>
+__global__ void __launch_bounds__(NG * AP_NC, AP_MINB) k_apply_banded(const ApplyArgs p) {
+  using PL = ApplyPlan<T, M0, MS, W, NG>;
+  constexpr int AP_BT = NG * AP_NC;
+  constexpr int ND = PL::ND, MAXM = PL::MAXM, XW = PL::XW, JC = AP_JC;
   if (p.guard == 1 && solver_idle(p.red.st)) return;
   if (p.guard == 2 && (p.red.st->stalled | (p.red.st->status != 0))) return;
 
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  cplx* stage_base = reinterpret_cast<cplx*>(smem_raw);
-  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)2 * PL::STAGE * sizeof(cplx));
+  ApplyCommon k;
+  k.stage_base = reinterpret_cast<cplx*>(smem_raw);
+  k.Ps = k.stage_base + (size_t)PL::NSTAGE * PL::STAGE;
+  k.full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)(PL::NSTAGE * PL::STAGE + PL::PS) * sizeof(cplx));
 
-  const int tid = threadIdx.x;
-  const int a0 = blockIdx.x * AP_NT;
-  const int a = a0 + tid;                                   // channel; lanes with a >= ld idle along
-  const int ld = p.ld, n_rad = p.n_rad;
-  const bool lane_ok = a < ld;
-  const int ac = lane_ok ? a : ld - 1;
-  const int i0 = blockIdx.y * p.seg_len;
-  const int i1 = min(n_rad, i0 + p.seg_len);
-  const int jlo = max(0, i0 - W), jhi = min(n_rad, i1 + W);   // input rows this segment needs
-  const int nchunks = (jhi - jlo + JC - 1) / JC;
+  const int grp = threadIdx.x / AP_NC;                       // warp-uniform
+  k.tid = threadIdx.x % AP_NC;
+  const int a0 = blockIdx.x * AP_NC;
+  k.a = a0 + k.tid;                                          // channel; lanes with a >= ld idle along
+  k.ld = p.ld; k.n_rad = p.n_rad;
+  k.lane_ok = k.a < k.ld;
+  k.ac = k.lane_ok ? k.a : k.ld - 1;
+  k.i0 = blockIdx.y * p.seg_len;
+  k.i1 = min(k.n_rad, k.i0 + p.seg_len);
+  k.jlo = max(0, k.i0 - W);
+  k.jhi = min(k.n_rad, k.i1 + W);                            // input rows [jlo, jhi) carry data
+  k.jend = k.i1 + W;                                         // rows [jhi, jend) only flush the output window
+  k.nchunks = (k.jend - k.jlo + JC - 1) / JC;
+  k.slot = p.slot[k.ac];                                     // index into this CTA's class list, or -1
+  k.blk_g = p.blk + (size_t)p.cls[k.ac] * k.n_rad * ND;      // global fallback for slot < 0
 
   // channel range of the x tile, clipped to the vector; the clipped cells stay zero (matching A entries are 0)
-  const int xa_lo = max(0, a0 - MAXM), xa_hi = min(ld, a0 + AP_NT + MAXM);
+  const int ld = k.ld, n_rad = k.n_rad, jlo = k.jlo, jhi = k.jhi;
+  const int xa_lo = max(0, a0 - MAXM), xa_hi = min(ld, a0 + AP_NC + MAXM);
   const int x_dst_off = xa_lo - (a0 - MAXM);
   const uint32_t x_bytes = (uint32_t)(xa_hi - xa_lo) * sizeof(cplx);
   const int* cta_cls = p.cta_cls + blockIdx.x * AP_MAXC;
+  cplx* stage_base = k.stage_base;
+  uint64_t* full = k.full;
 
   if (x_bytes != XW * sizeof(cplx)) {
-    for (int q = tid; q < 2 * PL::STAGE; q += AP_NT) stage_base[q] = make_double2(0, 0);
+    for (int q = threadIdx.x; q < PL::NSTAGE * PL::STAGE; q += AP_BT) stage_base[q] = make_double2(0, 0);
   }
-  if (tid == 0) {
-    mbar_init(&full[0], 1);
-    mbar_init(&full[1], 1);
+  if (threadIdx.x == 0) {
+    for (int q = 0; q < PL::NSTAGE; ++q) mbar_init(&full[q], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 
   auto issue = [&](int c) {                                  // one elected thread: all bulk copies of chunk c
-    cplx* st = stage_base + (size_t)(c & 1) * PL::STAGE;
-    uint64_t* bar = &full[c & 1];
+    cplx* st = stage_base + (size_t)(c % PL::NSTAGE) * PL::STAGE;
+    uint64_t* bar = &full[c % PL::NSTAGE];
     const int j = jlo + c * JC;
     const int nr = min(JC, jhi - j);
+    if (nr <= 0) return;                                     // a chunk of virtual rows only
     uint32_t bytes = (uint32_t)nr * x_bytes;
     int ncls = 0;
 #pragma unroll
@@ -127,115 +278,23 @@ __global__ void __launch_bounds__(AP_NT, 2) k_apply_banded(const ApplyArgs p) {
     if (T > 0) bulk_g2s(st, p.Rall + (size_t)j * T * ND, (uint32_t)nr * T * ND * sizeof(cplx), bar);
 #pragma unroll
     for (int q = 0; q < AP_MAXC; ++q) {
-      const int k = cta_cls[q];
-      if (k >= 0)
-        bulk_g2s(st + PL::RS + (size_t)q * JC * ND, p.blk + ((size_t)k * n_rad + j) * ND, (uint32_t)nr * ND * sizeof(cplx), bar);
+      const int kk = cta_cls[q];
+      if (kk >= 0)
+        bulk_g2s(st + PL::RS + (size_t)q * JC * ND, p.blk + ((size_t)kk * n_rad + j) * ND, (uint32_t)nr * ND * sizeof(cplx), bar);
     }
     for (int r = 0; r < nr; ++r)
       bulk_g2s(st + PL::RS + PL::BS + (size_t)r * XW + x_dst_off, p.x + (size_t)(j + r) * ld + xa_lo, x_bytes, bar);
   };
-  if (tid == 0) {
+  if (threadIdx.x == 0) {
     issue(0);
-    if (nchunks > 1) issue(1);
+    if (k.nchunks > 1) issue(1);
   }
 
-  // angular coefficients in registers, pre-multiplied by beta * g_L
-  cplx Areg[NS > 0 ? NS : 1];
-  if (T > 0) {
-    const double* g = p.g + (p.step_ptr ? (size_t)(*p.step_ptr) * T : 0);
-#pragma unroll
-    for (int L = 0; L < T; ++L) {
-      const double gl = g[L];
-      const cplx coef = make_double2(p.beta.x * gl, p.beta.y * gl);
-#pragma unroll
-      for (int q = 0; q < 2 * SH::m(L); ++q) {
-        const int s = SH::slot0(L) + q;
-        Areg[s] = cmul(coef, p.Aoff[(size_t)s * ld + ac]);
-      }
-    }
-  }
-  const int slot = p.slot[ac];                               // index into this CTA's class list, or -1
-  const cplx* blk_g = p.blk + (size_t)p.cls[ac] * n_rad * ND;   // global fallback for slot < 0
-
-  cplx yw[ND];
-#pragma unroll
-  for (int e = 0; e < ND; ++e) yw[e] = make_double2(0, 0);
   cplx d0 = make_double2(0, 0);
   double d1 = 0;
-
-  for (int c = 0; c < nchunks; ++c) {
-    const cplx* st = stage_base + (size_t)(c & 1) * PL::STAGE;
-    mbar_wait(&full[c & 1], (c >> 1) & 1);
-    const int jc0 = jlo + c * JC;
-    const int nr = min(JC, jhi - jc0);
-    for (int r = 0; r < nr; ++r) {
-      const int j = jc0 + r;
-      const int i = j - W;                                   // the output row completed by input row j
-      const bool emit = (i >= i0) && lane_ok;                // i < i1 always holds here
-      cplx ax = make_double2(0, 0);
-      if (emit && p.aux) ax = p.aux[(size_t)i * ld + a];
-      const cplx* xs = st + PL::RS + PL::BS + (size_t)r * XW + tid + MAXM;
-      const cplx x0 = xs[0];
-      if (slot >= 0) {
-        const cplx* bc = st + PL::RS + ((size_t)slot * JC + r) * ND;
-#pragma unroll
-        for (int e = 0; e < ND; ++e) cfma(yw[e], bc[e], x0);
-      } else {
-        const cplx* bc = blk_g + (size_t)j * ND;
-#pragma unroll
-        for (int e = 0; e < ND; ++e) cfma(yw[e], __ldg(bc + e), x0);
-      }
-      if (T > 0) {
-        cplx z[T > 0 ? T : 1];
-#pragma unroll
-        for (int L = 0; L < T; ++L) z[L] = make_double2(0, 0);
-#pragma unroll
-        for (int o = -MAXM; o <= MAXM; ++o) {
-          if (o == 0) continue;
-          const cplx xo = xs[o];
-#pragma unroll
-          for (int L = 0; L < T; ++L) {
-            if (SH::m(L) >= (o < 0 ? -o : o)) {
-              // slot order within a term: o = -m..-1 -> q = o + m ; o = 1..m -> q = m + o - 1
-              const int q = o < 0 ? o + SH::m(L) : SH::m(L) + o - 1;
-              cfma(z[L], Areg[SH::slot0(L) + q], xo);
-            }
-          }
-        }
-#pragma unroll
-        for (int L = 0; L < T; ++L) {
-          const cplx* rc = st + ((size_t)r * T + L) * ND;    // warp-uniform: broadcast LDS.128
-#pragma unroll
-          for (int e = 0; e < ND; ++e) cfma(yw[e], rc[e], z[L]);
-        }
-      }
-      if (emit) {
-        const cplx yv = yw[0];
-        p.y[(size_t)i * ld + a] = yv;
-        cfma_conj(d0, ax, yv);
-        d1 = fma(yv.x, yv.x, d1); d1 = fma(yv.y, yv.y, d1);
-      }
-#pragma unroll
-      for (int e = 0; e < ND - 1; ++e) yw[e] = yw[e + 1];
-      yw[ND - 1] = make_double2(0, 0);
-    }
-    __syncthreads();                                         // every warp is done with this stage
-    if (tid == 0 && c + 2 < nchunks) issue(c + 2);
-  }
-  // rows past the end of the matrix contribute nothing: flush the outputs still in the window
-  for (int j = jhi; j < i1 + W; ++j) {
-    const int i = j - W;
-    if (i >= i0 && lane_ok) {
-      const cplx yv = yw[0];
-      p.y[(size_t)i * ld + a] = yv;
-      if (p.aux) cfma_conj(d0, p.aux[(size_t)i * ld + a], yv);
-      d1 = fma(yv.x, yv.x, d1); d1 = fma(yv.y, yv.y, d1);
-    }
-#pragma unroll
-    for (int e = 0; e < ND - 1; ++e) yw[e] = yw[e + 1];
-    yw[ND - 1] = make_double2(0, 0);
-  }
-  if (p.red.fin != FIN_NONE) grid_reduce_finalize<AP_NT>(d0.x, d0.y, d1, p.red);
+  if (NG == 1 || grp == 0) apply_group<T, M0, MS, W, NG, 0>(p, k, issue, d0, d1);
+  else apply_group<T, M0, MS, W, NG, 1>(p, k, issue, d0, d1);
+  if (p.red.fin != FIN_NONE) grid_reduce_finalize<AP_BT>(d0.x, d0.y, d1, p.red);
 }
 
 // ---- generic path: arbitrary CSR A_L, arbitrary per-term bandwidths; one thread per output element. ----
@@ -297,19 +356,27 @@ bool apply_banded_available(int T, int m0, int mstep, int W) {
   return false;
 }
 
-int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, cudaStream_t s) {
-  dim3 grid((a.ld + AP_NT - 1) / AP_NT, (a.n_rad + a.seg_len - 1) / a.seg_len);
-#define X(t, aa, b, w) \
-  if (T == t && (t == 0 || (m0 == aa && mstep == b)) && W == w) {                                         \
-    static bool attr_set = false;                                                                         \
-    const size_t smem = ApplyPlan<t, aa, b, w>::SMEM;                                                     \
-    if (!attr_set) {                                                                                      \
-      if (cudaFuncSetAttribute(k_apply_banded<t, aa, b, w>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
-                               (int)smem) != cudaSuccess) return -2;                                      \
-      attr_set = true;                                                                                    \
-    }                                                                                                     \
-    k_apply_banded<t, aa, b, w><<<grid, AP_NT, smem, s>>>(a);                                             \
-    return 1;                                                                                             \
+template <int T, int M0, int MS, int W, int NG>
+static int launch_banded_one(const ApplyArgs& a, dim3 grid, cudaStream_t s) {
+  static bool attr_set = false;
+  const size_t smem = ApplyPlan<T, M0, MS, W, NG>::SMEM;
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(k_apply_banded<T, M0, MS, W, NG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
+        cudaSuccess)
+      return -2;
+    attr_set = true;
+  }
+  k_apply_banded<T, M0, MS, W, NG><<<grid, NG * AP_NC, smem, s>>>(a);
+  return 1;
+}
+
+// ng = number of warp groups the terms of a channel are split over (1 or 2); T == 0 always runs with one group.
+int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, int ng, cudaStream_t s) {
+  dim3 grid((a.ld + AP_NC - 1) / AP_NC, (a.n_rad + a.seg_len - 1) / a.seg_len);
+#define X(t, aa, b, w)                                                          \
+  if (T == t && (t == 0 || (m0 == aa && mstep == b)) && W == w) {               \
+    if (t == 0 || ng == 1) return launch_banded_one<t, aa, b, w, 1>(a, grid, s); \
+    return launch_banded_one<t, aa, b, w, (t == 0 ? 1 : 2)>(a, grid, s);         \
   }
   TDDE_BANDED_SHAPES(X)
 #undef X

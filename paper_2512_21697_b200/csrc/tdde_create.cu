@@ -127,12 +127,16 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
   h->path = detect_banded(&c, terms, &m0, &ms) ? 1 : 0;
   h->bT = T; h->bM0 = m0; h->bMS = ms; h->bW = w0;
   h->norm_banded = (h->path == 1);
+  // measured on B200 (Large T=5 and HBM-scale T=7): one group at 255 registers beats the two-group term split,
+  // whose 128-register budget makes ptxas spill; the split stays selectable for experiments
+  h->apply_ng = 1;
+  if (const char* env = std::getenv("TDDE_APPLY_NG")) h->apply_ng = std::atoi(env) == 2 ? 2 : 1;
 
-  // radial segment length (banded path): the kernel runs 2 CTAs per SM (296 slots on 148 SMs); every segment
+  // radial segment length (banded path): the kernel runs TDDE_AP_MINB CTAs per SM; every segment
   // recomputes 2 w0 halo rows.  Pick the segment count that minimises waves x (rows + halo).
   {
-    const int chan_blocks = (h->ld + 127) / 128;
-    const int slots = 148 * 2;
+    const int chan_blocks = (h->ld + TDDE_AP_NC - 1) / TDDE_AP_NC;
+    const int slots = 148 * TDDE_AP_MINB;
     long long best_cost = -1;
     int best_seg = n_rad;
     for (int segs = 1; segs <= n_rad; ++segs) {
@@ -255,11 +259,11 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
   }
   if (h->path == 1) {
     // per CTA (128 consecutive channels): the first TDDE_AP_MAXC distinct classes are staged in shared memory
-    const int n_cta = (h->ld + 127) / 128;
+    const int n_cta = (h->ld + TDDE_AP_NC - 1) / TDDE_AP_NC;
     std::vector<int> slot(h->ld, -1), cta_cls((size_t)n_cta * TDDE_AP_MAXC, -1);
     for (int b = 0; b < n_cta; ++b) {
       int cnt = 0;
-      for (int a = b * 128; a < std::min(h->ld, (b + 1) * 128); ++a) {
+      for (int a = b * TDDE_AP_NC; a < std::min(h->ld, (b + 1) * TDDE_AP_NC); ++a) {
         const int k = a < c.n_ang ? cls_of_chan[a] : 0;
         int q = 0;
         while (q < cnt && cta_cls[(size_t)b * TDDE_AP_MAXC + q] != k) ++q;

@@ -40,7 +40,7 @@ int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int b
     a.blk = blk_ptr(h, blk);
     a.Rall = h->d_Rall; a.slot = h->d_slot; a.cta_cls = h->d_cta_cls;
     a.Aoff = h->d_Aoff;
-    rc = launch_apply_banded(a, T, h->bM0, h->bMS, h->cfg.w0, h->stream);
+    rc = launch_apply_banded(a, T, h->bM0, h->bMS, h->cfg.w0, h->apply_ng, h->stream);
   } else {
     a.blk_row = blk_ptr(h, blk);
     for (int L = 0; L < T; ++L) {

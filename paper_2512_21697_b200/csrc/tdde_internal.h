@@ -13,7 +13,18 @@
 #define TDDE_MAX_TERMS 8
 #define TDDE_MAX_PARTIAL_BLOCKS 65536
 #define TDDE_TINY 1e-290
-#define TDDE_AP_JC 8
+#ifndef TDDE_AP_NC
+#define TDDE_AP_NC 128     // banded apply: channels per CTA
+#endif
+#ifndef TDDE_AP_MINB
+#define TDDE_AP_MINB 2     // banded apply: CTAs per SM the kernel is compiled for
+#endif
+#ifndef TDDE_AP_JC
+#define TDDE_AP_JC 4       // banded apply: radial rows per pipeline stage
+#endif
+#ifndef TDDE_AP_RU
+#define TDDE_AP_RU 2
+#endif
 #define TDDE_AP_MAXC 4
 #define TDDE_PC_MAXC 8
 #define TDDE_PC_MAXPARTS 16
@@ -119,7 +130,7 @@ struct PrecArgs {
 };
 
 // launchers (each returns the number of kernels launched, or -1 if no instantiation fits)
-int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, cudaStream_t s);
+int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, int ng, cudaStream_t s);
 bool apply_banded_available(int T, int m0, int mstep, int W);
 int launch_apply_generic(const ApplyArgs& a, cudaStream_t s);
 int launch_precond(const PrecArgs& a, cudaStream_t s);
