@@ -149,6 +149,10 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
       if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_seg = seg; }
     }
     h->seg_len = best_seg;
+    // the S-only apply has 13 complex FMAs per element: not ALU-bound, so halo recomputation is cheap and
+    // many short segments (about 4 waves of 3 CTAs per SM) hide the TMA latency instead
+    const int want = (4 * 148 * 3 + chan_blocks - 1) / chan_blocks;
+    h->seg_len_s = std::min(n_rad, std::max(4 * w0, (n_rad + want - 1) / want));
   }
 
   const zc* S = reinterpret_cast<const zc*>(S_band);

@@ -25,7 +25,7 @@ int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int b
   std::memset(&a, 0, sizeof(a));
   a.x = x; a.y = y; a.aux = aux;
   a.n_ang = h->cfg.n_ang; a.n_rad = h->cfg.n_rad; a.ld = h->ld;
-  a.seg_len = h->seg_len;
+  a.seg_len = (with_terms && h->cfg.n_terms > 0) ? h->seg_len : h->seg_len_s;
   a.cls = h->d_cls;
   a.beta = beta;
   a.g = g_dev; a.step_ptr = step_ptr;

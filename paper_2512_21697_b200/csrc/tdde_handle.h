@@ -19,6 +19,7 @@ struct tdde_handle {
   int path = 0;                  // 1 banded fast path, 0 generic
   int bT = 0, bM0 = 0, bMS = 0, bW = 0;
   int seg_len = 0;               // radial rows per thread (banded path)
+  int seg_len_s = 0;             // radial rows per thread for the S-only (T = 0) apply: latency-bound, wants more CTAs
   int apply_ng = 1;              // warp groups the terms are split over (banded path)
   bool norm_banded = false;      // S-only apply can use the banded T=0 kernel
 

@@ -25,7 +25,9 @@
 #ifndef TDDE_AP_RU
 #define TDDE_AP_RU 2
 #endif
-#define TDDE_AP_MAXC 4
+#ifndef TDDE_AP_MAXC
+#define TDDE_AP_MAXC 16    // banded apply: distinct kappa-classes per CTA staged in shared memory
+#endif
 #define TDDE_PC_MAXC 8
 #define TDDE_PC_MAXPARTS 16
 
