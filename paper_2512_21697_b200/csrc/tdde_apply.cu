@@ -214,7 +214,7 @@ __device__ __forceinline__ void apply_group(const ApplyArgs& p, const ApplyCommo
 }
 
 template <int T, int M0, int MS, int W, int NG>
-__global__ void __launch_bounds__(NG * AP_NC, AP_MINB) k_apply_banded(const ApplyArgs p) {
+__global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB)) k_apply_banded(const ApplyArgs p) {
   using PL = ApplyPlan<T, M0, MS, W, NG>;
   constexpr int AP_BT = NG * AP_NC;
   constexpr int ND = PL::ND, MAXM = PL::MAXM, XW = PL::XW, JC = AP_JC;

@@ -127,16 +127,17 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
   h->path = detect_banded(&c, terms, &m0, &ms) ? 1 : 0;
   h->bT = T; h->bM0 = m0; h->bMS = ms; h->bW = w0;
   h->norm_banded = (h->path == 1);
-  // measured on B200 (Large T=5 and HBM-scale T=7): one group at 255 registers beats the two-group term split,
-  // whose 128-register budget makes ptxas spill; the split stays selectable for experiments
-  h->apply_ng = 1;
+  // Term split over two warp groups (256-thread CTA, one per SM, 255 registers each): measured on B200 it wins once
+  // the per-thread A_L registers no longer fit (HBM-scale, T = 7: 3.21 -> 2.39 ms) and loses below (Large, T = 5:
+  // 0.31 -> 0.37 ms), so it is chosen by the number of terms.
+  h->apply_ng = (T >= 6) ? 2 : 1;
   if (const char* env = std::getenv("TDDE_APPLY_NG")) h->apply_ng = std::atoi(env) == 2 ? 2 : 1;
 
   // radial segment length (banded path): the kernel runs TDDE_AP_MINB CTAs per SM; every segment
   // recomputes 2 w0 halo rows.  Pick the segment count that minimises waves x (rows + halo).
   {
     const int chan_blocks = (h->ld + TDDE_AP_NC - 1) / TDDE_AP_NC;
-    const int slots = 148 * TDDE_AP_MINB;
+    const int slots = 148 * (h->apply_ng == 2 ? TDDE_AP_MINB2 : TDDE_AP_MINB);
     long long best_cost = -1;
     int best_seg = n_rad;
     for (int segs = 1; segs <= n_rad; ++segs) {

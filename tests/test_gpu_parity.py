@@ -277,3 +277,26 @@ def test_sampled_rows_at_bench_size_p10():
     del xd, z
     torch.cuda.empty_cache()
     prop.close()
+
+
+@pytest.mark.parametrize("ng", ["1", "2"])
+def test_apply_both_term_split_variants(ng, monkeypatch):
+    """The banded apply exists with one warp group and with the terms split over two; the library picks one by T.
+    Force each (TDDE_APPLY_NG is read at tdde_create) on a T = 7 and a T = 5 shape, ragged sizes."""
+    from paper_2512_21697_b200 import Tdde
+    monkeypatch.setenv("TDDE_APPLY_NG", ng)
+    for n_ang, n_r, T in [(150, 29, 7), (70, 41, 5)]:
+        p = tdde_inputs.make_synthetic(n_ang=n_ang, n_r=n_r, bandwidth=13, n_terms=T, dt=0.01, n_steps=2, rtol=1e-10,
+                                       seed=5, name="split", phase=np.pi / 2, e0=2.0)
+        prop = Tdde(p)
+        assert prop.apply_path == "banded"
+        ops, fact = orc.assemble(p), orc.factor_precond(p)
+        x = rand_vec(p.n, 2)
+        g = np.linspace(-1.0, 1.0, T)
+        y = prop.apply(1.0, 0.5j * p.dt, g, prop.to_device(x)).cpu().numpy()
+        assert rel(y, orc.apply(ops, 1.0, 0.5j * p.dt, g, x)) <= 1e-12
+        c = prop.to_device(p.c0)
+        prop.propagate(c, p.g_table(2))
+        c_ref, _ = orc.propagate(p, ops, fact, p.c0, 2)
+        assert rel(c.cpu().numpy(), c_ref) <= 1e-9
+        prop.close()
