@@ -191,8 +191,11 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
   {
     std::vector<zc> Sx(h->blk_count), Hx(h->blk_count), Mx(h->blk_count);
     std::vector<zc> Lc((size_t)c.n_cls * n_rad * w0), Uc((size_t)c.n_cls * n_rad * (w0 + 1));
-    // partition count of the preconditioner solve: about 1.5 warps per SM sub-partition (4 x 148), interiors >= 8 w0
-    int P = (int)((888 + h->ld / 32 - 1) / (h->ld / 32));
+    // partition count of the preconditioner solve: as many one-warp CTAs as are resident at once (shared memory of
+    // k_precond: 3 stages x 8 rows x (32 + TDDE_PC_MAXC (w0+1)) complex), never a nearly empty second wave
+    const size_t pc_smem = (size_t)3 * 8 * (32 + TDDE_PC_MAXC * (w0 + 1)) * 16 + 1024;
+    const int pc_slots = 148 * (int)std::min<size_t>(32, (227 * 1024) / pc_smem);
+    int P = std::max(1, pc_slots / (h->ld / 32));
     if (const char* env = std::getenv("TDDE_PC_PARTS")) P = std::atoi(env);
     const bool templated_w = (w0 == 3 || w0 == 6 || w0 == 9 || w0 == 13);
     P = templated_w ? std::min(std::max(P, 1), TDDE_PC_MAXPARTS) : 1;
@@ -262,8 +265,9 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     if (rc) return rc;
     CU(cudaStreamSynchronize(s));
   }
-  if (h->path == 1) {
+  {
     // per CTA (128 consecutive channels): the first TDDE_AP_MAXC distinct classes are staged in shared memory
+    // (used by the banded apply and by the preconditioner's correction kernel)
     const int n_cta = (h->ld + TDDE_AP_NC - 1) / TDDE_AP_NC;
     std::vector<int> slot(h->ld, -1), cta_cls((size_t)n_cta * TDDE_AP_MAXC, -1);
     for (int b = 0; b < n_cta; ++b) {
@@ -279,6 +283,10 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     int rc;
     if ((rc = dev_upload(&h->d_slot, slot.data(), slot.size(), s))) return rc;
     if ((rc = dev_upload(&h->d_cta_cls, cta_cls.data(), cta_cls.size(), s))) return rc;
+    CU(cudaStreamSynchronize(s));
+  }
+  if (h->path == 1) {
+    int rc;
     const int nd = 2 * w0 + 1;
     std::vector<zc> Rall((size_t)n_rad * std::max(T, 1) * nd), Rc((size_t)n_rad * nd);
     for (int L = 0; L < T; ++L) {

@@ -63,7 +63,7 @@ int enqueue_precond(tdde_handle* h, const cplx* x, cplx* y, const SolverState* s
   p.P = h->pc_P; p.ns = h->pc_ns;
   for (int q = 0; q <= TDDE_PC_MAXPARTS; ++q) p.range_lo[q] = h->pc_range_lo[q];
   for (int q = 0; q < TDDE_PC_MAXPARTS; ++q) p.int_hi[q] = h->pc_int_hi[q];
-  p.Esp = h->d_Esp; p.Msep = h->d_Msep; p.Scinv = h->d_Scinv; p.rs = h->d_rs;
+  p.Esp = h->d_Esp; p.Msep = h->d_Msep; p.Scinv = h->d_Scinv; p.rs = h->d_rs; p.aslot = h->d_slot; p.cta_cls = h->d_cta_cls;
   int rc = launch_precond(p, h->stream);
   if (rc == -2) return tdde_cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(precond)");
   if (rc < 0) return TDDE_EINVAL;

@@ -129,6 +129,8 @@ struct PrecArgs {
   const cplx* Msep;        // [n_cls][ns][2w+1]
   const cplx* Scinv;       // [n_cls][ns][ns]
   cplx* rs;                // scratch [ns][ld]: Schur right-hand side
+  const int* aslot;        // [ld] the apply's per-CTA class slot (128-channel groups), used by k_precond_correct
+  const int* cta_cls;      // [n_cta][TDDE_AP_MAXC]
   const SolverState* st;   // nullable guard
 };
 

@@ -211,33 +211,61 @@ __global__ void __launch_bounds__(128) k_precond_schur_mul(const PrecArgs p) {
 }
 
 // ---- kernel C: x_I = t_I - E^- x_S(before) - E^+ x_S(after): streaming, 2 W complex FMAs per row ----
-#define PCC_ROWS 64
+// CTA = 128 channels x PCC_ROWS interior rows.  The spike rows of the CTA's kappa-classes (same class list as the
+// operator apply) are staged in shared memory with cp.async and read back as warp-broadcasts; each thread first
+// issues all of its vector loads, so enough bytes are in flight to stream at HBM speed.
+#define PCC_ROWS 16
 template <int W>
 __global__ void __launch_bounds__(128) k_precond_correct(const PrecArgs p) {
   if (p.st && solver_idle(p.st)) return;
-  const int a = blockIdx.x * 128 + threadIdx.x;
-  if (a >= p.ld) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx* Es = reinterpret_cast<cplx*>(smem_raw);                     // [TDDE_AP_MAXC][PCC_ROWS][2W]
   const int q = blockIdx.y, ld = p.ld;
   const int lo = p.range_lo[q], hi = p.int_hi[q];
-  const int i0 = lo + blockIdx.z * PCC_ROWS, i1 = min(hi, i0 + PCC_ROWS);
+  const int i0 = lo + blockIdx.z * PCC_ROWS;
   if (i0 >= hi) return;
-  const int k = p.cls[a];
+  const int nr = min(PCC_ROWS, hi - i0);
+  const int a = blockIdx.x * 128 + threadIdx.x;
+  const bool ok = a < ld;
+  const int ac = ok ? a : ld - 1;
+  const int* ccls = p.cta_cls + blockIdx.x * TDDE_AP_MAXC;
+  for (int s = 0; s < TDDE_AP_MAXC; ++s) {
+    const int k = ccls[s];
+    if (k < 0) break;
+    const cplx* src = p.Esp + ((size_t)k * p.n_rad + i0) * 2 * W;
+    cplx* dst = Es + (size_t)s * PCC_ROWS * 2 * W;
+    for (int e = threadIdx.x; e < nr * 2 * W; e += 128) cp_async16(dst + e, src + e);
+  }
+  cp_async_commit();
+  cplx t[PCC_ROWS];
+#pragma unroll
+  for (int r = 0; r < PCC_ROWS; ++r) t[r] = (r < nr) ? p.y[(size_t)(i0 + r) * ld + ac] : make_double2(0, 0);
   cplx xm[W], xp[W];
 #pragma unroll
   for (int c = 0; c < W; ++c) {
-    xm[c] = q > 0 ? p.y[(size_t)(p.int_hi[q - 1] + c) * ld + a] : make_double2(0, 0);
-    xp[c] = q + 1 < p.P ? p.y[(size_t)(hi + c) * ld + a] : make_double2(0, 0);
+    xm[c] = q > 0 ? p.y[(size_t)(p.int_hi[q - 1] + c) * ld + ac] : make_double2(0, 0);
+    xp[c] = q + 1 < p.P ? p.y[(size_t)(hi + c) * ld + ac] : make_double2(0, 0);
     xm[c] = make_double2(-xm[c].x, -xm[c].y);
     xp[c] = make_double2(-xp[c].x, -xp[c].y);
   }
-  const cplx* E = p.Esp + (size_t)k * p.n_rad * 2 * W;
-#pragma unroll 2
-  for (int i = i0; i < i1; ++i) {
-    cplx t = p.y[(size_t)i * ld + a];
-    const cplx* e = E + (size_t)i * 2 * W;
+  cp_async_wait<0>();
+  __syncthreads();
+  const int slot = p.aslot[ac];
+  const cplx* Eg = p.Esp + ((size_t)p.cls[ac] * p.n_rad + i0) * 2 * W;
+  const cplx* El = Es + (size_t)(slot >= 0 ? slot : 0) * PCC_ROWS * 2 * W;
 #pragma unroll
-    for (int c = 0; c < W; ++c) { cfma(t, __ldg(e + c), xm[c]); cfma(t, __ldg(e + W + c), xp[c]); }
-    p.y[(size_t)i * ld + a] = t;
+  for (int r = 0; r < PCC_ROWS; ++r) {
+    if (r < nr) {
+      cplx v = t[r];
+      if (slot >= 0) {
+#pragma unroll
+        for (int c = 0; c < W; ++c) { cfma(v, El[r * 2 * W + c], xm[c]); cfma(v, El[r * 2 * W + W + c], xp[c]); }
+      } else {
+#pragma unroll
+        for (int c = 0; c < W; ++c) { cfma(v, __ldg(Eg + r * 2 * W + c), xm[c]); cfma(v, __ldg(Eg + r * 2 * W + W + c), xp[c]); }
+      }
+      if (ok) p.y[(size_t)(i0 + r) * ld + a] = v;
+    }
   }
 }
 
@@ -275,8 +303,11 @@ template <int W>
 static int launch_precond_w(const PrecArgs& a, cudaStream_t s) {
   static bool attr_set = false;
   const size_t smem = PrecPlan<W>::SMEM;
+  const size_t csmem = (size_t)TDDE_AP_MAXC * PCC_ROWS * 2 * W * sizeof(cplx);
+  static_assert(TDDE_AP_NC == 128, "k_precond_correct shares the apply's 128-channel class lists");
   if (!attr_set) {
     if (cudaFuncSetAttribute(k_precond<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -2;
+    if (cudaFuncSetAttribute(k_precond_correct<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)csmem) != cudaSuccess) return -2;
     attr_set = true;
   }
   k_precond<W><<<dim3(a.ld / PC_NT, a.P), PC_NT, smem, s>>>(a);
@@ -285,7 +316,7 @@ static int launch_precond_w(const PrecArgs& a, cudaStream_t s) {
   k_precond_schur_mul<W><<<dim3((a.ld + 127) / 128, a.ns), 128, 0, s>>>(a);
   int max_int = 0;
   for (int q = 0; q < a.P; ++q) max_int = max_int > a.int_hi[q] - a.range_lo[q] ? max_int : a.int_hi[q] - a.range_lo[q];
-  k_precond_correct<W><<<dim3((a.ld + 127) / 128, a.P, (max_int + PCC_ROWS - 1) / PCC_ROWS), 128, 0, s>>>(a);
+  k_precond_correct<W><<<dim3((a.ld + 127) / 128, a.P, (max_int + PCC_ROWS - 1) / PCC_ROWS), 128, csmem, s>>>(a);
   return 4;
 }
 
