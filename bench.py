@@ -211,6 +211,11 @@ def ours_main(args):
         flops_apply = 8.0 * F * nint
         sm_max = float(peaks.get("sm_max_mhz", 1965.0))
         fp64_peak_nominal = NUM_SMS * FP64_FMA_PER_CLK_PER_SM * 2 * sm_max * 1e6
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "r01_traffic.json")      # dram bytes of one ncu --set full capture
+        if os.path.exists(tpath):
+            with open(tpath) as f:
+                traffic = json.load(f).get(args.config, {}).get("dram_bytes_per_launch")
         t_apply = kt["apply"] * 1e-3
         ach = flops_apply / t_apply / 1e12
         hbm = float(peaks["hbm_gbs"])
@@ -236,7 +241,8 @@ def ours_main(args):
                     "note": "one tdde_propagate_host call of K steps: state vector H2D + g table H2D + K steps + state D2H"},
             "roofline": {"bound": "alu", "kernel": "k_apply_banded (v = A y with fused <rhat,v>)",
                          "achieved": ach, "peak": fp64_peak_nominal / 1e12, "unit": "TFLOP/s",
-                         "frac": ach / (fp64_peak_nominal / 1e12), "traffic": None,
+                         "frac": ach / (fp64_peak_nominal / 1e12), "traffic": traffic,
+                         "algorithmic_bytes_per_launch": 48 * nint,
                          "peak_kind": "derived: 148 SMs x 64 DFMA/clk x 2 x %.0f MHz" % sm_max,
                          "fp64_peak_measured_tflops": fp64_peak_meas / 1e12,
                          "frac_of_measured_dfma": ach / (fp64_peak_meas / 1e12),
@@ -245,7 +251,7 @@ def ours_main(args):
             "kernels": kernels,
         }
         if world == 1 and not args.no_cpu_baseline:
-            cb, _ = run_oracle(args.config, 2, 0, args.sample_ang)
+            cb, _ = run_oracle(args.config, 4, 0, args.sample_ang)
             line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
         print(json.dumps(line))
     prop.close()
@@ -262,7 +268,7 @@ def main():
     ap.add_argument("--config", default="hbm", choices=sorted(tdde_inputs.CONFIGS))
     ap.add_argument("--phase", type=float, default=0.0, help="phase of g(t) = E0 sin(w t + phase); 0 = BASELINE config")
     ap.add_argument("--kernel-reps", type=int, default=10)
-    ap.add_argument("--sample-ang", type=int, default=12, help="angular channels of the oracle's bounded sample")
+    ap.add_argument("--sample-ang", type=int, default=24, help="angular channels of the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -126,6 +126,12 @@ int tdde_step_forced(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, int32
 int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, const double* g, double* ms_out);
 int tdde_fp64_peak(void* cuda_stream, double* flops_out);
 
+/* Host-only self-test of the set-up code behind tdde_precond (no GPU needed): builds a random banded
+ * M = S + i tau H of size n and half-bandwidth w, the partitioned factors for P partitions, replays the
+ * solve on the host and writes the relative residual ||M y - b|| / ||b|| to *rel_res (host).  Returns the number of
+ * partitions actually used (>= 1; the plan shrinks P until interiors are >= 8 w rows) or a negative tdde_status. */
+int tdde_selftest_partition(int32_t n, int32_t w, int32_t P, uint32_t seed, double* rel_res);
+
 /* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
 int64_t tdde_launch_count(const tdde_handle* h);
 

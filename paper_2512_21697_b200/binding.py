@@ -19,7 +19,7 @@ LIB_PATH = os.environ.get("TDDE_LIB_PATH", os.path.join(_HERE, "libtdde.so"))
 EXPORTS = [
     "tdde_create", "tdde_step", "tdde_propagate", "tdde_norm", "tdde_apply", "tdde_precond",
     "tdde_propagate_host", "tdde_step_forced", "tdde_time_kernel", "tdde_fp64_peak", "tdde_launch_count",
-    "tdde_apply_path", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
+    "tdde_apply_path", "tdde_selftest_partition", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
 ]
 
 STATUS = {0: "TDDE_OK", -1: "TDDE_EINVAL", -2: "TDDE_ENOMEM", -3: "TDDE_ECUDA", -4: "TDDE_ESINGULAR",
@@ -81,6 +81,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.tdde_launch_count.argtypes = [vp]
     lib.tdde_launch_count.restype = i64
     lib.tdde_apply_path.argtypes = [vp]
+    lib.tdde_selftest_partition.argtypes = [i32, i32, i32, C.c_uint32, C.POINTER(dbl)]
+    lib.tdde_selftest_partition.restype = C.c_int
     lib.tdde_destroy.argtypes = [vp]
     lib.tdde_destroy.restype = None
     lib.tdde_strerror.argtypes = [C.c_int]

@@ -113,3 +113,35 @@ def test_product_does_not_import_oracle():
         if f.endswith(".py"):
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "paper_2512_21697_b200" not in txt and "libtdde" not in txt, f
+
+
+@pytest.mark.parametrize("n,w,P", [(128, 3, 4), (400, 13, 3), (2000, 6, 9), (4000, 6, 3), (97, 3, 16), (64, 9, 1),
+                                   (1000, 9, 7), (50, 6, 8)])
+def test_partitioned_factorisation_host(lib, n, w, P):
+    """Host set-up of the partitioned preconditioner solve (tdde_partition.cu) replayed on the host: the result must
+    solve the original banded system to rounding, for ragged sizes, every templated bandwidth, and plans that shrink."""
+    res = C.c_double()
+    used = lib.tdde_selftest_partition(n, w, P, 7, C.byref(res))
+    assert 1 <= used <= P
+    if (n - (P - 1) * w) // P >= 8 * w:
+        assert used == P
+    assert res.value < 1e-13, (n, w, P, used, res.value)
+
+
+def test_reference_arm_prints_on_rank0_only():
+    """bench.py --impl reference under a 2-rank launch: rank 0 prints the JSON line, other ranks exit 0 silently."""
+    import json
+    import subprocess
+    import sys
+    env = dict(os.environ, WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT="29533")
+    outs = []
+    for rank in (0, 1):
+        r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
+                            "--warmup", "0", "--config", "tiny", "--sample-ang", "4"], env=dict(env, RANK=str(rank), LOCAL_RANK=str(rank)),
+                           capture_output=True, text=True, timeout=600)
+        assert r.returncode == 0, r.stderr[-500:]
+        outs.append(r.stdout.strip())
+    line = json.loads(outs[0].splitlines()[-1])
+    assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
+    assert line["e2e"]["h2d_bytes_per_step"] == 0
+    assert outs[1] == ""
