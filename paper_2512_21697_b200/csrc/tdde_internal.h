@@ -19,8 +19,10 @@
 #ifndef TDDE_AP_MINB
 #define TDDE_AP_MINB 2     // banded apply: CTAs per SM the kernel is compiled for
 #endif
-#ifndef TDDE_AP_JC
+#ifndef TDDE_AP_MINB2
 #define TDDE_AP_MINB2 1    // CTAs per SM for the two-group (256-thread) variant
+#endif
+#ifndef TDDE_AP_JC
 #define TDDE_AP_JC 4       // banded apply: radial rows per pipeline stage
 #endif
 #ifndef TDDE_AP_RU
