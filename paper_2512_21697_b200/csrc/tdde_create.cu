@@ -192,8 +192,8 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     std::vector<zc> Sx(h->blk_count), Hx(h->blk_count), Mx(h->blk_count);
     std::vector<zc> Lc((size_t)c.n_cls * n_rad * w0), Uc((size_t)c.n_cls * n_rad * (w0 + 1));
     // partition count of the preconditioner solve: as many one-warp CTAs as are resident at once (shared memory of
-    // k_precond: 3 stages x 8 rows x (32 + TDDE_PC_MAXC (w0+1)) complex), never a nearly empty second wave
-    const size_t pc_smem = (size_t)3 * 8 * (32 + TDDE_PC_MAXC * (w0 + 1)) * 16 + 1024;
+    // k_precond: 3 stages x 8 rows x TDDE_PC_MAXC (w0+1) complex), never a nearly empty second wave
+    const size_t pc_smem = (size_t)3 * 8 * (TDDE_PC_MAXC * (w0 + 1)) * 16 + 1024;
     const int pc_slots = 148 * (int)std::min<size_t>(32, (227 * 1024) / pc_smem);
     int P = std::max(1, pc_slots / (h->ld / 32));
     if (const char* env = std::getenv("TDDE_PC_PARTS")) P = std::atoi(env);

@@ -138,11 +138,11 @@ static void fill_stats(const tdde_handle* h, tdde_stats* st) {
 
 // X (internal layout) holds c; advance n_steps steps.  Always ends with one state read.
 static int run_steps(tdde_handle* h, long long n_steps) {
-  const long long batch = 64;
   long long enq = 0;          // steps enqueued so far (== steps_done when nothing stalled)
   int rc;
   h->launches += launch_step_open(h->d_st, 0, 0, 0, h->stream);
   while (true) {
+    const long long batch = h->nspec_learned ? 64 : 4;      // short batches until nspec has settled
     const long long upto = std::min(n_steps, enq + batch);
     for (; enq < upto; ++enq) {
       if ((rc = enqueue_step_start(h))) return rc;
@@ -168,6 +168,7 @@ static int run_steps(tdde_handle* h, long long n_steps) {
       }
       enq = h->h_st->steps_done;      // steps after the stalled one were no-ops: redo them
     }
+    if (!h->h_st->stalled && h->h_st->steps_done >= upto) h->nspec_learned = true;
     if (h->h_st->steps_done >= n_steps) return 0;
     enq = h->h_st->steps_done;
   }

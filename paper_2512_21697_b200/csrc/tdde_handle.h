@@ -56,7 +56,8 @@ struct tdde_handle {
   long long g_cap = 0;
   double* d_g_small = nullptr;               // [T] for tdde_apply
   double* d_zero_g = nullptr;                // [T] zeros
-  int nspec = 2;                             // speculated iterations per step
+  int nspec = 1;                             // speculated iterations per step (grows when a step stalls)
+  bool nspec_learned = false;                // first batches are short until one has passed without a stall
   long long launches = 0;
 };
 

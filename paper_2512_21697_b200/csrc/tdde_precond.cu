@@ -29,12 +29,13 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 template <int W>
 struct PrecPlan {
   static constexpr int CW = W + 1;                                   // coefficient row width (U needs W+1)
-  static constexpr int XS = PC_ROWS * PC_NT;                         // complex per stage
-  static constexpr int CS = PC_MAXC * PC_ROWS * CW;
-  static constexpr int STAGE = XS + CS;
+  static constexpr int STAGE = PC_MAXC * PC_ROWS * CW;               // complex per stage (factor rows only)
   static constexpr size_t SMEM = (size_t)PC_STAGES * STAGE * sizeof(cplx);
 };
 
+// Kernel A of the partitioned solve (and the whole solve when P == 1): one warp = 32 channels x one row range.
+// Factor rows of the warp's kappa-classes stream through a cp.async ring in shared memory; the vector rows of the
+// next stage are prefetched into registers while the current stage is being solved.
 template <int W>
 __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
   using PL = PrecPlan<W>;
@@ -47,8 +48,8 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
   // rows [row0, row0 + n_rad): interior blockIdx.y plus the separator after it (identity rows in the factors)
   const int row0 = p.range_lo[blockIdx.y];
   const int n_rad = p.range_lo[blockIdx.y + 1] - row0;
-  const cplx* xin = p.x + (size_t)row0 * ld;
-  cplx* yout = p.y + (size_t)row0 * ld;
+  const cplx* xin = p.x + (size_t)row0 * ld + a;
+  cplx* yout = p.y + (size_t)row0 * ld + a;
   const int* wcls = p.warp_cls + blockIdx.x * PC_MAXC;
   int ncls = 0;
 #pragma unroll
@@ -58,17 +59,17 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
   const int nst = (n_rad + PC_ROWS - 1) / PC_ROWS;
 
   cplx pw[W + 1];
+  cplx xn[PC_ROWS];
 
   // ================= forward: L y = x =================
   {
-    auto issue = [&](int s) {                                        // rows [s*R, s*R + R)
+    auto issue = [&](int s) {                                        // factor rows [s*R, s*R + R) of every class
       if (s < nst) {
         cplx* st = ring + (size_t)(s % PC_STAGES) * PL::STAGE;
         const int r0 = s * PC_ROWS, nr = min(PC_ROWS, n_rad - r0);
-        for (int r = 0; r < nr; ++r) cp_async16(st + r * PC_NT + lane, xin + (size_t)(r0 + r) * ld + a);
         for (int q = 0; q < ncls; ++q) {
           const cplx* src = p.Lcol + ((size_t)wcls[q] * n_tot + row0 + r0) * W;
-          cplx* dst = st + PL::XS + (size_t)q * PC_ROWS * PL::CW;
+          cplx* dst = st + (size_t)q * PC_ROWS * PL::CW;
           for (int e = lane; e < nr * W; e += PC_NT) cp_async16(dst + e, src + e);
         }
       }
@@ -77,40 +78,49 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
 #pragma unroll
     for (int d = 0; d <= W; ++d) pw[d] = make_double2(0, 0);
     for (int s = 0; s < PC_STAGES - 1; ++s) issue(s);
+#pragma unroll
+    for (int r = 0; r < PC_ROWS; ++r) xn[r] = xin[(size_t)min(r, n_rad - 1) * ld];
     for (int s = 0; s < nst; ++s) {
+      const int r0 = s * PC_ROWS, nr = min(PC_ROWS, n_rad - r0);
+      cplx xc[PC_ROWS];
+#pragma unroll
+      for (int r = 0; r < PC_ROWS; ++r) xc[r] = xn[r];
+      if (s + 1 < nst) {
+#pragma unroll
+        for (int r = 0; r < PC_ROWS; ++r) xn[r] = xin[(size_t)min(r0 + PC_ROWS + r, n_rad - 1) * ld];
+      }
       issue(s + PC_STAGES - 1);
       cp_async_wait<PC_STAGES - 1>();
       __syncwarp();
-      const cplx* st = ring + (size_t)(s % PC_STAGES) * PL::STAGE;
-      const int r0 = s * PC_ROWS, nr = min(PC_ROWS, n_rad - r0);
-      const cplx* cs = st + PL::XS + (size_t)(slot >= 0 ? slot : 0) * PC_ROWS * PL::CW;
+      const cplx* cs = ring + (size_t)(s % PC_STAGES) * PL::STAGE + (size_t)(slot >= 0 ? slot : 0) * PC_ROWS * PL::CW;
       const cplx* cg = p.Lcol + ((size_t)k * n_tot + row0 + r0) * W;
-#pragma unroll 4
-      for (int r = 0; r < nr; ++r) {
-        const cplx xi = st[r * PC_NT + lane];
-        cplx c[W];
-        if (slot >= 0) {
 #pragma unroll
-          for (int d = 0; d < W; ++d) c[d] = cs[r * W + d];
-        } else {
+      for (int r = 0; r < PC_ROWS; ++r) {
+        if (r < nr) {
+          const cplx xi = xc[r];
+          cplx c[W];
+          if (slot >= 0) {
 #pragma unroll
-          for (int d = 0; d < W; ++d) c[d] = __ldg(cg + r * W + d);
+            for (int d = 0; d < W; ++d) c[d] = cs[r * W + d];
+          } else {
+#pragma unroll
+            for (int d = 0; d < W; ++d) c[d] = __ldg(cg + r * W + d);
+          }
+          const cplx nc0 = make_double2(-c[0].x, -c[0].y);
+          cplx base = pw[1];
+          cfma(base, nc0, xi);                                       // off the chain
+          const cplx yi = cadd(xi, pw[0]);
+          yout[(size_t)(r0 + r) * ld] = yi;
+          const cplx nyi = make_double2(-yi.x, -yi.y);
+          cfma(base, nc0, pw[0]);                                    // the chain: one complex FMA per row
+          pw[0] = base;
+#pragma unroll
+          for (int d = 1; d < W; ++d) { pw[d] = pw[d + 1]; cfma(pw[d], c[d], nyi); }
         }
-        const cplx nc0 = make_double2(-c[0].x, -c[0].y);
-        cplx base = pw[1];
-        cfma(base, nc0, xi);                                         // off the chain
-        const cplx yi = cadd(xi, pw[0]);
-        yout[(size_t)(r0 + r) * ld + a] = yi;
-        const cplx nyi = make_double2(-yi.x, -yi.y);
-        cfma(base, nc0, pw[0]);                                      // the chain: one complex FMA per row
-        pw[0] = base;
-#pragma unroll
-        for (int d = 1; d < W; ++d) { pw[d] = pw[d + 1]; cfma(pw[d], c[d], nyi); }
       }
       __syncwarp();
     }
     cp_async_wait<0>();
-    __threadfence();   // the U sweep re-reads, asynchronously, what this thread just stored
   }
   // ================= backward: U x = y (rows descending; stage s covers rows [n_rad - (s+1) R, n_rad - s R)) ====
   {
@@ -118,10 +128,9 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
       if (s < nst) {
         cplx* st = ring + (size_t)(s % PC_STAGES) * PL::STAGE;
         const int hi = n_rad - s * PC_ROWS, lo = max(0, hi - PC_ROWS), nr = hi - lo;
-        for (int r = 0; r < nr; ++r) cp_async16(st + r * PC_NT + lane, yout + (size_t)(lo + r) * ld + a);
         for (int q = 0; q < ncls; ++q) {
           const cplx* src = p.Ucol + ((size_t)wcls[q] * n_tot + row0 + lo) * (W + 1);
-          cplx* dst = st + PL::XS + (size_t)q * PC_ROWS * PL::CW;
+          cplx* dst = st + (size_t)q * PC_ROWS * PL::CW;
           for (int e = lane; e < nr * (W + 1); e += PC_NT) cp_async16(dst + e, src + e);
         }
       }
@@ -130,36 +139,48 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
 #pragma unroll
     for (int d = 0; d <= W; ++d) pw[d] = make_double2(0, 0);
     for (int s = 0; s < PC_STAGES - 1; ++s) issue(s);
+    // xn[r] holds row (hi - 1 - r) of the stage: the order in which the sweep consumes them
+#pragma unroll
+    for (int r = 0; r < PC_ROWS; ++r) xn[r] = yout[(size_t)max(n_rad - 1 - r, 0) * ld];
     for (int s = 0; s < nst; ++s) {
+      const int hi = n_rad - s * PC_ROWS, lo = max(0, hi - PC_ROWS), nr = hi - lo;
+      cplx xc[PC_ROWS];
+#pragma unroll
+      for (int r = 0; r < PC_ROWS; ++r) xc[r] = xn[r];
+      if (s + 1 < nst) {
+#pragma unroll
+        for (int r = 0; r < PC_ROWS; ++r) xn[r] = yout[(size_t)max(lo - 1 - r, 0) * ld];
+      }
       issue(s + PC_STAGES - 1);
       cp_async_wait<PC_STAGES - 1>();
       __syncwarp();
-      const cplx* st = ring + (size_t)(s % PC_STAGES) * PL::STAGE;
-      const int hi = n_rad - s * PC_ROWS, lo = max(0, hi - PC_ROWS), nr = hi - lo;
-      const cplx* cs = st + PL::XS + (size_t)(slot >= 0 ? slot : 0) * PC_ROWS * PL::CW;
+      const cplx* cs = ring + (size_t)(s % PC_STAGES) * PL::STAGE + (size_t)(slot >= 0 ? slot : 0) * PC_ROWS * PL::CW;
       const cplx* cg = p.Ucol + ((size_t)k * n_tot + row0 + lo) * (W + 1);
-#pragma unroll 4
-      for (int r = nr - 1; r >= 0; --r) {
-        const cplx yi = st[r * PC_NT + lane];
-        cplx c[W + 1];
-        if (slot >= 0) {
 #pragma unroll
-          for (int d = 0; d <= W; ++d) c[d] = cs[r * (W + 1) + d];
-        } else {
+      for (int rr = 0; rr < PC_ROWS; ++rr) {
+        if (rr < nr) {
+          const int r = nr - 1 - rr;                                 // row lo + r, factor row r of the stage
+          const cplx yi = xc[rr];
+          cplx c[W + 1];
+          if (slot >= 0) {
 #pragma unroll
-          for (int d = 0; d <= W; ++d) c[d] = __ldg(cg + r * (W + 1) + d);
+            for (int d = 0; d <= W; ++d) c[d] = cs[r * (W + 1) + d];
+          } else {
+#pragma unroll
+            for (int d = 0; d <= W; ++d) c[d] = __ldg(cg + r * (W + 1) + d);
+          }
+          // x_i = uinv (y_i + pw0);  pw0' = pw1 - U[i-1][i] x_i = (pw1 - c1 y_i) - c1 pw0  with c1 = U[i-1][i] uinv
+          const cplx nc1 = make_double2(-c[1].x, -c[1].y);
+          cplx base = pw[1];
+          cfma(base, nc1, yi);                                       // off the chain
+          const cplx xi = cmul(cadd(yi, pw[0]), c[0]);
+          yout[(size_t)(lo + r) * ld] = xi;
+          const cplx nxi = make_double2(-xi.x, -xi.y);
+          cfma(base, nc1, pw[0]);                                    // the chain
+          pw[0] = base;
+#pragma unroll
+          for (int d = 1; d < W; ++d) { pw[d] = pw[d + 1]; cfma(pw[d], c[d + 1], nxi); }
         }
-        // x_i = uinv (y_i + pw0);  pw0' = pw1 - U[i-1][i] x_i = (pw1 - c1 y_i) - c1 pw0  with c1 = U[i-1][i] uinv
-        const cplx nc1 = make_double2(-c[1].x, -c[1].y);
-        cplx base = pw[1];
-        cfma(base, nc1, yi);                                         // off the chain
-        const cplx xi = cmul(cadd(yi, pw[0]), c[0]);
-        yout[(size_t)(lo + r) * ld + a] = xi;
-        const cplx nxi = make_double2(-xi.x, -xi.y);
-        cfma(base, nc1, pw[0]);                                      // the chain
-        pw[0] = base;
-#pragma unroll
-        for (int d = 1; d < W; ++d) { pw[d] = pw[d + 1]; cfma(pw[d], c[d + 1], nxi); }
       }
       __syncwarp();
     }
