@@ -107,6 +107,8 @@ extern "C" void tdde_destroy(tdde_handle* h) {
     if (h->d_Acol[L]) cudaFree(h->d_Acol[L]);
     if (h->d_Aval[L]) cudaFree(h->d_Aval[L]);
   }
+  if (h->step_exec) cudaGraphExecDestroy(h->step_exec);
+  if (h->cap) cudaStreamDestroy(h->cap);
   if (h->h_st) cudaFreeHost(h->h_st);
   cudaGetLastError();
   delete h;

@@ -7,6 +7,7 @@
 // finds out at its next state read (once per batch of steps), resumes that step with more iterations and
 // raises nspec.  All BiCGSTAB scalars stay in SolverState on the device.
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 #include "tdde_handle.h"
 
@@ -119,11 +120,14 @@ static int enqueue_iteration(tdde_handle* h) {
 
 static int upload_g(tdde_handle* h, const double* g_table, long long n_steps) {
   const int T = h->cfg.n_terms;
+  const long long n_req = n_steps;
   if (T == 0) { if (!h->d_g) { CU(cudaMalloc((void**)&h->d_g, sizeof(double))); h->g_cap = 1; } return 0; }
   if (n_steps > h->g_cap) {
+    n_steps = std::max<long long>(n_steps, 4096);       // generous: a new table address would force a re-capture
     if (h->d_g) { CU(cudaStreamSynchronize(h->stream)); cudaFree(h->d_g); h->d_g = nullptr; }
     CU(cudaMalloc((void**)&h->d_g, (size_t)n_steps * T * sizeof(double)));
     h->g_cap = n_steps;
+    n_steps = n_req;
   }
   CU(cudaMemcpyAsync(h->d_g, g_table, (size_t)n_steps * T * sizeof(double), cudaMemcpyHostToDevice, h->stream));
   return 0;
@@ -136,6 +140,50 @@ static void fill_stats(const tdde_handle* h, tdde_stats* st) {
   st->rel_res = s->last_rel_res; st->status = s->status; st->last_half_iters = s->last_half_iters;
 }
 
+static int enqueue_step_raw(tdde_handle* h) {
+  int rc;
+  if ((rc = enqueue_step_start(h))) return rc;
+  for (int it = 0; it < h->nspec; ++it)
+    if ((rc = enqueue_iteration(h))) return rc;
+  h->launches += launch_step_close(h->d_st, h->stream);
+  return 0;
+}
+
+// One step as a CUDA graph.  The sequence is identical for every step (the g row is picked by the device-side step
+// counter), so it is captured once and replayed; any failure falls back to plain launches for good.
+static bool ensure_graph(tdde_handle* h) {
+  static const bool disabled = std::getenv("TDDE_NO_GRAPH") != nullptr;
+  if (disabled || !h->graph_ok || !h->nspec_learned) return false;
+  if (!h->step_exec || h->graph_nspec != h->nspec || h->graph_g != h->d_g) {
+    if (h->step_exec) { cudaGraphExecDestroy(h->step_exec); h->step_exec = nullptr; }
+    if (!h->cap && cudaStreamCreateWithFlags(&h->cap, cudaStreamNonBlocking) != cudaSuccess) { h->graph_ok = false; cudaGetLastError(); return false; }
+    cudaStream_t user = h->stream;
+    const long long l0 = h->launches;
+    cudaGraph_t g = nullptr;
+    bool ok = cudaStreamBeginCapture(h->cap, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+    if (ok) {
+      h->stream = h->cap;
+      ok = enqueue_step_raw(h) == 0;
+      h->stream = user;
+      ok = (cudaStreamEndCapture(h->cap, &g) == cudaSuccess) && ok && g;
+    }
+    h->graph_launches = h->launches - l0;
+    h->launches = l0;
+    if (ok) ok = cudaGraphInstantiate(&h->step_exec, g, 0) == cudaSuccess;
+    if (g) cudaGraphDestroy(g);
+    if (!ok) { h->graph_ok = false; h->step_exec = nullptr; cudaGetLastError(); return false; }
+    h->graph_nspec = h->nspec; h->graph_g = h->d_g;
+  }
+  return true;
+}
+
+static int enqueue_step(tdde_handle* h) {
+  if (!ensure_graph(h)) return enqueue_step_raw(h);
+  CU(cudaGraphLaunch(h->step_exec, h->stream));
+  h->launches += h->graph_launches;
+  return 0;
+}
+
 // X (internal layout) holds c; advance n_steps steps.  Always ends with one state read.
 static int run_steps(tdde_handle* h, long long n_steps) {
   long long enq = 0;          // steps enqueued so far (== steps_done when nothing stalled)
@@ -145,10 +193,7 @@ static int run_steps(tdde_handle* h, long long n_steps) {
     const long long batch = h->nspec_learned ? 64 : 4;      // short batches until nspec has settled
     const long long upto = std::min(n_steps, enq + batch);
     for (; enq < upto; ++enq) {
-      if ((rc = enqueue_step_start(h))) return rc;
-      for (int it = 0; it < h->nspec; ++it)
-        if ((rc = enqueue_iteration(h))) return rc;
-      h->launches += launch_step_close(h->d_st, h->stream);
+      if ((rc = enqueue_step(h))) return rc;
     }
     if ((rc = sync_state(h))) return rc;
     CU(cudaGetLastError());
@@ -169,7 +214,7 @@ static int run_steps(tdde_handle* h, long long n_steps) {
       enq = h->h_st->steps_done;      // steps after the stalled one were no-ops: redo them
     }
     if (!h->h_st->stalled && h->h_st->steps_done >= upto) h->nspec_learned = true;
-    if (h->h_st->steps_done >= n_steps) return 0;
+    if (h->h_st->steps_done >= n_steps) { ensure_graph(h); return 0; }   // capture now, outside the next call's steps
     enq = h->h_st->steps_done;
   }
 }

@@ -59,6 +59,14 @@ struct tdde_handle {
   int nspec = 1;                             // speculated iterations per step (grows when a step stalls)
   bool nspec_learned = false;                // first batches are short until one has passed without a stall
   long long launches = 0;
+  // CUDA graph of one step (start + nspec iterations + close): captured once on an internal stream, replayed on the
+  // caller's stream; re-captured when nspec or the device g table changes
+  cudaStream_t cap = nullptr;
+  cudaGraphExec_t step_exec = nullptr;
+  int graph_nspec = -1;
+  const double* graph_g = nullptr;
+  long long graph_launches = 0;
+  bool graph_ok = true;
 };
 
 extern thread_local std::string g_last_cuda_error;
