@@ -300,3 +300,35 @@ def test_apply_both_term_split_variants(ng, monkeypatch):
         c_ref, _ = orc.propagate(p, ops, fact, p.c0, 2)
         assert rel(c.cpu().numpy(), c_ref) <= 1e-9
         prop.close()
+
+
+def test_sampled_rows_and_properties_at_hbm_scale():
+    """BASELINE configs[4] (HBM-scale, the workload bench.py times, two-warp-group apply): sampled outputs against the
+    oracle's direct summation, M (M^-1 x) = x, and after 3 CN steps S-norm conservation and the solver's residual."""
+    import torch
+    p, prop = make("hbm", with_c0=False)
+    assert prop.apply_path == "banded"
+    x = rand_vec(p.n, 33)
+    xd = prop.to_device(x)
+    g = np.linspace(-1.0, 1.0, p.n_terms)
+    y = prop.apply(1.0, 0.5j * p.dt, g, xd).cpu().numpy().reshape(p.n_ang, p.n_rad)
+    rng = np.random.default_rng(1)
+    ns = 300
+    chan = np.concatenate([rng.integers(0, p.n_ang, ns), [0, 0, p.n_ang - 1, p.n_ang - 1, 3, 7, 127, 128, p.n_ang - 8]])
+    rad = np.concatenate([rng.integers(0, p.n_rad, ns), [0, p.n_rad - 1, 0, p.n_rad - 1, 5, 6, 443, 444, p.n_rad - 7]])
+    ref = orc.apply_rows_sampled(p, 1.0, 0.5j * p.dt, g, x, chan, rad)
+    scale = np.sqrt(np.mean(np.abs(ref) ** 2))
+    assert np.max(np.abs(y[chan, rad] - ref)) / scale <= 1e-12
+    del y
+    z = prop.precond(xd)
+    back = prop.apply(1.0, 0.5j * p.dt, np.zeros(p.n_terms), z)
+    err = float(torch.linalg.vector_norm(back - xd) / torch.linalg.vector_norm(xd))
+    assert err <= 1e-12
+    del z, back
+    n0 = prop.norm(xd)
+    st = prop.propagate(xd, p.g_table(3))
+    assert st["steps"] == 3 and st["status"] == 0 and st["rel_res"] <= p.rtol
+    assert abs(prop.norm(xd) / n0 - 1.0) <= 30 * p.rtol
+    del xd
+    torch.cuda.empty_cache()
+    prop.close()
