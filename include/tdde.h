@@ -86,12 +86,14 @@ int tdde_create(tdde_handle** out, const tdde_config* cfg, const tdde_c64* S_ban
                 const int32_t* cls_of_chan, const tdde_term* terms, void* cuda_stream);
 
 /* One CN step in place on c_dev (device, n complex128).  g_mid: host [n_terms], g_L(t_{n+1/2}).
- * If st != NULL the call synchronises the stream and fills *st; otherwise solver failures are latched and
- * returned by the next synchronising call.  On failure c_dev holds the last iterate. */
+ * The call synchronises the stream once at its end (the speculative step driver must learn whether a step ran out
+ * of enqueued iterations) and returns the step's status; *st (nullable) receives the statistics.  There is no host
+ * synchronisation per BiCGSTAB iteration.  On failure c_dev holds the last iterate. */
 int tdde_step(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, tdde_stats* st);
 
 /* n_steps CN steps in place on c_dev.  g_table: host [n_steps][n_terms], row s = g_L at the midpoint of step s.
- * Stops at the first failing step (st->steps tells how many completed).  Synchronises iff st != NULL. */
+ * Stops at the first failing step (st->steps tells how many completed).  Device state is read back once per batch
+ * of 64 steps and once at the end; the call returns synchronised.  st is nullable. */
 int tdde_propagate(tdde_handle* h, tdde_c64* c_dev, int64_t n_steps, const double* g_table, tdde_stats* st);
 
 /* *out (host) = Re(c^H S c), the total probability in the non-orthogonal basis (S: PAPER.md:178-182).
