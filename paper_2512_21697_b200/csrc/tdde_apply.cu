@@ -62,7 +62,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 //   Bs[MAXC][JC][ND]  block column coefficients of the (at most MAXC) distinct kappa-classes of this CTA
 //   Xs[JC][XW]        x rows of the CTA's 128 channels plus MAXM halo channels on each side (one bulk copy per row)
 // plus Ps[2][JC][128]: partial outputs handed from warp group 1 to warp group 0 (double-buffered).
-template <int T, int M0, int MS, int W, int NG>
+template <int T, int M0, int MS, int W, int NG, bool BLK>
 struct ApplyPlan {
   using SH = BandShape<T, M0, MS>;
   static constexpr int ND = 2 * W + 1;
@@ -71,11 +71,11 @@ struct ApplyPlan {
   // rows per stage: the two-group variant (one CTA per SM) takes twice as many when the shared memory allows,
   // which halves the number of CTA barriers (measured: HBM-scale 2.41 -> 2.25 ms)
   __host__ __device__ static constexpr size_t smem_for(int jc) {
-    return (size_t)(3 * (jc * T * ND + AP_MAXC * jc * ND + jc * XW) + ((T > 0 && NG == 2) ? 2 * jc * AP_NC : 0)) * sizeof(cplx) + 64;
+    return (size_t)(3 * (jc * T * ND + (BLK ? AP_MAXC * jc * ND : 0) + jc * XW) + ((T > 0 && NG == 2) ? 2 * jc * AP_NC : 0)) * sizeof(cplx) + 64;
   }
   static constexpr int JC = (NG == 2 && smem_for(2 * AP_JC) <= 220 * 1024) ? 2 * AP_JC : AP_JC;
   static constexpr int RS = JC * T * ND;                    // complex elements
-  static constexpr int BS = AP_MAXC * JC * ND;
+  static constexpr int BS = BLK ? AP_MAXC * JC * ND : 0;   // no block part: no class coefficients staged
   static constexpr int XS = JC * XW;
   static constexpr int STAGE = RS + BS + XS;
   static constexpr int PS = (T > 0 && NG == 2) ? 2 * JC * AP_NC : 0;
@@ -86,7 +86,7 @@ struct ApplyPlan {
   // write-out and the fused inner products.  Greedy balance of complex FMAs per row, largest term first.
   __host__ __device__ static constexpr int cost(int L) { return ND + 2 * SH::m(L); }
   __host__ __device__ static constexpr int mask() {          // bit L set: term L belongs to group 1
-    int c0 = ND + 4, c1 = 0, mk = 0;
+    int c0 = (BLK ? ND : 0) + 4, c1 = 0, mk = 0;
     for (int L = T - 1; L >= 0; --L) {
       if (c1 < c0) { c1 += cost(L); mk |= 1 << L; } else c0 += cost(L);
     }
@@ -110,10 +110,10 @@ struct ApplyCommon {
 };
 
 // Work of one warp group G over the whole radial segment (see k_apply_banded).
-template <int T, int M0, int MS, int W, int NG, int G, class IssueFn>
+template <int T, int M0, int MS, int W, int NG, bool BLK, int G, class IssueFn>
 __device__ __forceinline__ void apply_group(const ApplyArgs& p, const ApplyCommon& k, IssueFn issue, cplx& d0, double& d1) {
   using SH = BandShape<T, M0, MS>;
-  using PL = ApplyPlan<T, M0, MS, W, NG>;
+  using PL = ApplyPlan<T, M0, MS, W, NG, BLK>;
   constexpr int ND = PL::ND, MAXM = PL::MAXM, NS = SH::nslots(), XW = PL::XW, JC = PL::JC, GM = PL::gmaxm(G);
   constexpr bool SPLIT = (NG == 2) && (T > 0);
   constexpr int RU = TDDE_AP_RU;                             // rows unrolled together (register pressure vs ILP)
@@ -159,10 +159,11 @@ __device__ __forceinline__ void apply_group(const ApplyArgs& p, const ApplyCommo
         if (G == 0) {
           if (emit && p.aux) ax = p.aux[(size_t)i * ld + k.a];
           if (SPLIT) pg = ps[r * AP_NC + k.tid];
+          if (!BLK && emit) pg = cadd(pg, p.addv[(size_t)i * ld + k.a]);   // block part replaced by a known vector
         }
         if (r < nr_real) {
           const cplx* xs = st + PL::RS + PL::BS + (size_t)r * XW + k.tid + MAXM;
-          if (G == 0) {
+          if (G == 0 && BLK) {
             const cplx x0 = xs[0];
             if (k.slot >= 0) {
               const cplx* bc = st + PL::RS + ((size_t)k.slot * JC + r) * ND;
@@ -219,9 +220,9 @@ __device__ __forceinline__ void apply_group(const ApplyArgs& p, const ApplyCommo
   }
 }
 
-template <int T, int M0, int MS, int W, int NG>
+template <int T, int M0, int MS, int W, int NG, bool BLK>
 __global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB)) k_apply_banded(const ApplyArgs p) {
-  using PL = ApplyPlan<T, M0, MS, W, NG>;
+  using PL = ApplyPlan<T, M0, MS, W, NG, BLK>;
   constexpr int AP_BT = NG * AP_NC;
   constexpr int ND = PL::ND, MAXM = PL::MAXM, XW = PL::XW, JC = PL::JC;
   if (p.guard == 1 && solver_idle(p.red.st)) return;
@@ -276,15 +277,17 @@ __global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB
     if (nr <= 0) return;                                     // a chunk of virtual rows only
     uint32_t bytes = (uint32_t)nr * x_bytes;
     int ncls = 0;
+    if (BLK) {
 #pragma unroll
-    for (int q = 0; q < AP_MAXC; ++q) ncls += (cta_cls[q] >= 0);
+      for (int q = 0; q < AP_MAXC; ++q) ncls += (cta_cls[q] >= 0);
+    }
     bytes += (uint32_t)ncls * nr * ND * sizeof(cplx);
     if (T > 0) bytes += (uint32_t)nr * T * ND * sizeof(cplx);
     mbar_expect_tx(bar, bytes);
     if (T > 0) bulk_g2s(st, p.Rall + (size_t)j * T * ND, (uint32_t)nr * T * ND * sizeof(cplx), bar);
 #pragma unroll
     for (int q = 0; q < AP_MAXC; ++q) {
-      const int kk = cta_cls[q];
+      const int kk = BLK ? cta_cls[q] : -1;
       if (kk >= 0)
         bulk_g2s(st + PL::RS + (size_t)q * JC * ND, p.blk + ((size_t)kk * n_rad + j) * ND, (uint32_t)nr * ND * sizeof(cplx), bar);
     }
@@ -298,8 +301,8 @@ __global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB
 
   cplx d0 = make_double2(0, 0);
   double d1 = 0;
-  if (NG == 1 || grp == 0) apply_group<T, M0, MS, W, NG, 0>(p, k, issue, d0, d1);
-  else apply_group<T, M0, MS, W, NG, 1>(p, k, issue, d0, d1);
+  if (NG == 1 || grp == 0) apply_group<T, M0, MS, W, NG, BLK, 0>(p, k, issue, d0, d1);
+  else apply_group<T, M0, MS, W, NG, BLK, 1>(p, k, issue, d0, d1);
   if (p.red.fin != FIN_NONE) grid_reduce_finalize<AP_BT>(d0.x, d0.y, d1, p.red);
 }
 
@@ -362,17 +365,17 @@ bool apply_banded_available(int T, int m0, int mstep, int W) {
   return false;
 }
 
-template <int T, int M0, int MS, int W, int NG>
+template <int T, int M0, int MS, int W, int NG, bool BLK>
 static int launch_banded_one(const ApplyArgs& a, dim3 grid, cudaStream_t s) {
   static bool attr_set = false;
-  const size_t smem = ApplyPlan<T, M0, MS, W, NG>::SMEM;
+  const size_t smem = ApplyPlan<T, M0, MS, W, NG, BLK>::SMEM;
   if (!attr_set) {
-    if (cudaFuncSetAttribute(k_apply_banded<T, M0, MS, W, NG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
+    if (cudaFuncSetAttribute(k_apply_banded<T, M0, MS, W, NG, BLK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
         cudaSuccess)
       return -2;
     attr_set = true;
   }
-  k_apply_banded<T, M0, MS, W, NG><<<grid, NG * AP_NC, smem, s>>>(a);
+  k_apply_banded<T, M0, MS, W, NG, BLK><<<grid, NG * AP_NC, smem, s>>>(a);
   return 1;
 }
 
@@ -381,8 +384,11 @@ int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, int
   dim3 grid((a.ld + AP_NC - 1) / AP_NC, (a.n_rad + a.seg_len - 1) / a.seg_len);
 #define X(t, aa, b, w)                                                          \
   if (T == t && (t == 0 || (m0 == aa && mstep == b)) && W == w) {               \
-    if (t == 0 || ng == 1) return launch_banded_one<t, aa, b, w, 1>(a, grid, s); \
-    return launch_banded_one<t, aa, b, w, (t == 0 ? 1 : 2)>(a, grid, s);         \
+    if (t == 0) return launch_banded_one<t, aa, b, w, 1, true>(a, grid, s);                                      \
+    if (a.addv) return ng == 1 ? launch_banded_one<t, aa, b, w, 1, (t == 0)>(a, grid, s)                         \
+                               : launch_banded_one<t, aa, b, w, (t == 0 ? 1 : 2), (t == 0)>(a, grid, s);         \
+    return ng == 1 ? launch_banded_one<t, aa, b, w, 1, true>(a, grid, s)                                         \
+                   : launch_banded_one<t, aa, b, w, (t == 0 ? 1 : 2), true>(a, grid, s);                         \
   }
   TDDE_BANDED_SHAPES(X)
 #undef X

@@ -21,10 +21,11 @@ static const cplx* blk_ptr(const tdde_handle* h, int blk) {
 }
 
 int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int blk, cplx beta, bool with_terms,
-                  const double* g_dev, const int* step_ptr, int guard, int fin, SolverState* st) {
+                  const double* g_dev, const int* step_ptr, int guard, int fin, SolverState* st, const cplx* addv) {
   ApplyArgs a;
   std::memset(&a, 0, sizeof(a));
   a.x = x; a.y = y; a.aux = aux;
+  a.addv = (h->path == 1 && with_terms && h->cfg.n_terms > 0) ? addv : nullptr;
   a.n_ang = h->cfg.n_ang; a.n_rad = h->cfg.n_rad; a.ld = h->ld;
   a.seg_len = (with_terms && h->cfg.n_terms > 0) ? h->seg_len : h->seg_len_s;
   a.cls = h->d_cls;
@@ -103,17 +104,19 @@ static int enqueue_step_start(tdde_handle* h) {
 }
 
 // One full BiCGSTAB iteration in the order of SURVEY 8(c) C4.
+// Banded path: since y = M^-1 p, A y = (M + i tau sum_L g_L A_L (x) R_L) y = p + i tau (coupling terms) y up to the rounding
+// of the solve, so the two applies of the iteration skip the block part and add p (resp. s) instead.
 static int enqueue_iteration(tdde_handle* h) {
   SolverState* st = h->d_st;
   const cplx itau = make_double2(0.0, h->tau);
   int rc;
   h->launches += launch_vec_p(make_vec_args(h, st, FIN_NONE), h->stream);                 // p = r + beta (p - omega v)
   if ((rc = enqueue_precond(h, h->p, h->y, st))) return rc;                               // y = M^-1 p
-  if ((rc = enqueue_apply(h, h->y, h->v, h->rhat, BLK_MP, itau, true, h->d_g, &st->step_idx, 1, FIN_ALPHA, st))) return rc;
+  if ((rc = enqueue_apply(h, h->y, h->v, h->rhat, BLK_MP, itau, true, h->d_g, &st->step_idx, 1, FIN_ALPHA, st, h->p))) return rc;
   h->launches += launch_vec_s(make_vec_args(h, st, FIN_S), h->stream);                    // s = r - alpha v, ||s||
   h->launches += launch_vec_halfexit(make_vec_args(h, st, FIN_NONE), h->stream);          // x += alpha y on the ||s|| exit
   if ((rc = enqueue_precond(h, h->s, h->z, st))) return rc;                               // z = M^-1 s
-  if ((rc = enqueue_apply(h, h->z, h->t, h->s, BLK_MP, itau, true, h->d_g, &st->step_idx, 1, FIN_OMEGA, st))) return rc;
+  if ((rc = enqueue_apply(h, h->z, h->t, h->s, BLK_MP, itau, true, h->d_g, &st->step_idx, 1, FIN_OMEGA, st, h->s))) return rc;
   h->launches += launch_vec_xr(make_vec_args(h, st, FIN_R), h->stream);                   // x, r updates, ||r||, <rhat,r>
   return 0;
 }

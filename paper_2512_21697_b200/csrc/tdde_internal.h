@@ -83,6 +83,7 @@ struct ApplyArgs {
   const cplx* x;           // internal layout
   cplx* y;
   const cplx* aux;         // vector for the fused dot (nullable)
+  const cplx* addv;        // banded path, nullable: y = addv + (coupling terms only) x; the block part is skipped
   int n_ang, n_rad, ld;
   int seg_len;             // radial rows per thread
   const int* cls;          // [ld] class per channel (pads: class 0)
