@@ -199,6 +199,13 @@ def ours_main(args):
     kt = {name: prop.time_kernel(which, reps, g_mid) for which, name in
           [(0, "apply"), (1, "precond"), (2, "vec_p"), (3, "vec_s"), (4, "vec_xr"), (5, "transpose"), (6, "apply_S")]}
     fp64_peak_meas = prop.fp64_peak()
+    pv = None
+    if args.paper_variant and prop.apply_path == "banded":
+        xv = prop.to_device(p.c0)
+        _, ta, ts, nnz = prop.paper_variant(g_mid, xv, reps=3)
+        pv = {"nnz": nnz, "assemble_ms": ta, "spmv_ms": ts, "spmv_GBps": 20.0 * nnz / (ts * 1e-3) / 1e9,
+              "note": "paper's formulation on this GPU (PAPER.md:301-305): one CSR assembly per step, one SpMV per apply"}
+        del xv
     clocks = sampler.result()
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
@@ -261,6 +268,7 @@ def ours_main(args):
                          "cfma_per_element": F, "flops_per_launch": flops_apply,
                          "alg_hbm_GBps": kernels["apply"]["alg_GBps"], "hbm_peak_GBps": hbm, "hbm_peak_kind": peak_kind},
             "kernels": kernels,
+            "paper_variant": pv,
         }
         if world == 1 and not args.no_cpu_baseline:
             cb, _ = run_oracle(args.config, 4, 0, args.sample_ang)
@@ -282,6 +290,8 @@ def main():
     ap.add_argument("--kernel-reps", type=int, default=10)
     ap.add_argument("--sample-ang", type=int, default=24, help="angular channels of the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--paper-variant", action="store_true",
+                    help="also time the paper's formulation (CSR assembly + SpMV) on this GPU; needs 20 B per non-zero")
     args = ap.parse_args()
     if args.impl == "reference":
         reference_main(args)

@@ -128,6 +128,15 @@ int tdde_step_forced(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, int32
 int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, const double* g, double* ms_out);
 int tdde_fp64_peak(void* cuda_stream, double* flops_out);
 
+/* Comparator, not on the product path: the paper's own formulation on this GPU.  Allocates the global
+ * CSR matrix A = S + i dt/2 H(g) (structure once), recomputes every non-zero from the stored radial and
+ * angular matrices with one assembly kernel and forms y = A x by CSR SpMV, `reps` times
+ * each; mean milliseconds go to *ms_assemble / *ms_spmv (host, nullable), the non-zero count to *nnz (host, nullable).
+ * x_dev, y_dev: device, n complex128, boundary layout, must not alias.  Needs 20 bytes of device memory per non-zero.
+ * Only for problems on the banded apply path (tdde_apply_path == 1), else TDDE_EINVAL.  Synchronises. */
+int tdde_paper_variant(tdde_handle* h, const double* g, const tdde_c64* x_dev, tdde_c64* y_dev, int32_t reps,
+                       double* ms_assemble, double* ms_spmv, int64_t* nnz);
+
 /* Host-only self-test of the set-up code behind tdde_precond (no GPU needed): builds a random banded
  * M = S + i tau H of size n and half-bandwidth w, the partitioned factors for P partitions, replays the
  * solve on the host and writes the relative residual ||M y - b|| / ||b|| to *rel_res (host).  Returns the number of

@@ -19,7 +19,7 @@ LIB_PATH = os.environ.get("TDDE_LIB_PATH", os.path.join(_HERE, "libtdde.so"))
 EXPORTS = [
     "tdde_create", "tdde_step", "tdde_propagate", "tdde_norm", "tdde_apply", "tdde_precond",
     "tdde_propagate_host", "tdde_step_forced", "tdde_time_kernel", "tdde_fp64_peak", "tdde_launch_count",
-    "tdde_apply_path", "tdde_selftest_partition", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
+    "tdde_apply_path", "tdde_selftest_partition", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
 ]
 
 STATUS = {0: "TDDE_OK", -1: "TDDE_EINVAL", -2: "TDDE_ENOMEM", -3: "TDDE_ECUDA", -4: "TDDE_ESINGULAR",
@@ -83,6 +83,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.tdde_apply_path.argtypes = [vp]
     lib.tdde_selftest_partition.argtypes = [i32, i32, i32, C.c_uint32, C.POINTER(dbl)]
     lib.tdde_selftest_partition.restype = C.c_int
+    lib.tdde_paper_variant.argtypes = [vp, vp, vp, vp, i32, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i64)]
+    lib.tdde_paper_variant.restype = C.c_int
     lib.tdde_destroy.argtypes = [vp]
     lib.tdde_destroy.restype = None
     lib.tdde_strerror.argtypes = [C.c_int]
@@ -222,6 +224,16 @@ class Tdde:
         out = C.c_double()
         _check(self.lib, self.lib.tdde_time_kernel(self.h, which, reps, _np_ptr(garr), C.byref(out)), "tdde_time_kernel")
         return out.value
+
+    def paper_variant(self, g, x_dev, reps: int = 3):
+        """The paper's formulation (CSR assembly + SpMV) as a comparator: returns (y, ms_assemble, ms_spmv, nnz)."""
+        garr = _g_array(g, self.n_terms) if self.n_terms else np.zeros(1)
+        y = self.torch.empty_like(x_dev)
+        ta, ts, nnz = C.c_double(), C.c_double(), C.c_int64()
+        rc = self.lib.tdde_paper_variant(self.h, _np_ptr(garr), self._vec(x_dev, "x"), self._vec(y, "y"), reps,
+                                         C.byref(ta), C.byref(ts), C.byref(nnz))
+        _check(self.lib, rc, "tdde_paper_variant")
+        return y, ta.value, ts.value, nnz.value
 
     def fp64_peak(self) -> float:
         out = C.c_double()
