@@ -28,6 +28,9 @@ import tdde_inputs  # noqa: E402
 METRIC = "cn_time_steps_per_s"
 UNIT = "steps/s"
 NUM_SMS = 148
+# dram__bytes_read.sum + dram__bytes_write.sum of one operator-apply launch, from one `ncu --set full` capture
+# (profiles/r01_apply_hbm_ncu.txt); bench.py cannot run ncu itself, so other configs report null
+MEASURED_DRAM_BYTES_PER_APPLY = {"hbm": 1.654e9}
 FP64_FMA_PER_CLK_PER_SM = 64          # B200: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2 TFLOP/s nominal
 
 
@@ -230,11 +233,7 @@ def ours_main(args):
         flops_apply = 8.0 * F * nint
         sm_max = float(peaks.get("sm_max_mhz", 1965.0))
         fp64_peak_nominal = NUM_SMS * FP64_FMA_PER_CLK_PER_SM * 2 * sm_max * 1e6
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "r01_traffic.json")      # dram bytes of one ncu --set full capture
-        if os.path.exists(tpath):
-            with open(tpath) as f:
-                traffic = json.load(f).get(args.config, {}).get("dram_bytes_per_launch")
+        traffic = MEASURED_DRAM_BYTES_PER_APPLY.get(args.config)
         t_apply = kt["apply"] * 1e-3
         ach = flops_apply / t_apply / 1e12
         hbm = float(peaks["hbm_gbs"])
