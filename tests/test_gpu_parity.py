@@ -345,3 +345,35 @@ def test_paper_variant_matches_oracle(smallmed, tiny):
         # union pattern of the assembled matrix: (coupled channels) x (band) per row, as SURVEY C2 counts it
         A = (ops.S + 0.5j * p.dt * (ops.H0 + sum(ops.K))).tocsr()
         assert nnz >= A.nnz and ta > 0 and ts > 0
+
+
+def test_eigenstate_phase_closed_form_p3_on_gpu(hyd):
+    """P3 on the CUDA path itself (no oracle in the loop): H0 v = E S v  =>  after N field-free CN steps
+    c = ((1 - i tau E) / (1 + i tau E))^N v exactly, and every step takes the ||s|| exit at half-iteration 1."""
+    import scipy.linalg as sla
+    p, prop, _, _ = hyd
+    S, H = p.meta["dense"][2]                     # kappa = +2 block (3d3/2-like), a state other than the fixture's 1s
+    E, V = sla.eigh(H, S)
+    j = int(np.nonzero(E > -p.meta["c"] ** 2)[0][0]) + 1
+    a = p.meta["chans"].index((2, 0.5))
+    c0 = np.zeros(p.n, dtype=np.complex128)
+    c0[a * p.n_rad:(a + 1) * p.n_rad] = V[:, j]
+    N = 20
+    c = prop.to_device(c0)
+    st = prop.propagate(c, np.zeros((N, p.n_terms)))
+    tau = 0.5 * p.dt
+    phase = ((1 - 1j * tau * E[j]) / (1 + 1j * tau * E[j])) ** N
+    assert rel(c.cpu().numpy(), phase * c0) <= 1e-9
+    assert st["half_iters"] == N
+
+
+def test_breakdown_is_reported_for_non_finite_input(tiny):
+    p, prop, _, _ = tiny
+    bad = p.c0.copy()
+    bad[7] = np.nan
+    c = prop.to_device(bad)
+    st = prop.propagate(c, p.g_table(2), check=False)
+    assert st["rc"] == -5 and st["steps"] == 0
+    c = prop.to_device(p.c0)                      # the handle recovers on the next call
+    st = prop.propagate(c, p.g_table(2))
+    assert st["steps"] == 2 and st["status"] == 0
