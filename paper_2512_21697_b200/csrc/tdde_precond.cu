@@ -85,7 +85,11 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
       cplx xc[PC_ROWS];
 #pragma unroll
       for (int r = 0; r < PC_ROWS; ++r) xc[r] = xn[r];
-      if (s + 1 < nst) {
+      if (r0 + 2 * PC_ROWS <= n_rad) {                               // next stage is full: no clamping
+        const cplx* xp = xin + (size_t)(r0 + PC_ROWS) * ld;
+#pragma unroll
+        for (int r = 0; r < PC_ROWS; ++r) { xn[r] = *xp; xp += ld; }
+      } else if (s + 1 < nst) {
 #pragma unroll
         for (int r = 0; r < PC_ROWS; ++r) xn[r] = xin[(size_t)min(r0 + PC_ROWS + r, n_rad - 1) * ld];
       }
@@ -147,7 +151,11 @@ __global__ void __launch_bounds__(PC_NT) k_precond(const PrecArgs p) {
       cplx xc[PC_ROWS];
 #pragma unroll
       for (int r = 0; r < PC_ROWS; ++r) xc[r] = xn[r];
-      if (s + 1 < nst) {
+      if (lo >= PC_ROWS) {                                           // next stage is full: no clamping
+        const cplx* xp = yout + (size_t)(lo - 1) * ld;
+#pragma unroll
+        for (int r = 0; r < PC_ROWS; ++r) { xn[r] = *xp; xp -= ld; }
+      } else if (s + 1 < nst) {
 #pragma unroll
         for (int r = 0; r < PC_ROWS; ++r) xn[r] = yout[(size_t)max(lo - 1 - r, 0) * ld];
       }
