@@ -204,9 +204,14 @@ __device__ __forceinline__ void apply_group(const ApplyArgs& p, const ApplyCommo
         if (G == 1) {
           if (SPLIT) ps[r * AP_NC + k.tid] = yw[0];
         } else if (emit) {
-          const cplx yv = cadd(yw[0], pg);
-          p.y[(size_t)i * ld + k.a] = yv;
-          cfma_conj(d0, ax, yv);
+          cplx yv = cadd(yw[0], pg);
+          if (p.emode == 2) {                                 // ||b||^2 = ||S c + r0 / 2||^2, nothing stored
+            yv.x = fma(0.5, ax.x, yv.x); yv.y = fma(0.5, ax.y, yv.y);
+          } else {
+            if (p.emode == 1) { yv = cmul(p.oscale, yv); p.y2[(size_t)i * ld + k.a] = yv; }
+            p.y[(size_t)i * ld + k.a] = yv;
+            cfma_conj(d0, ax, yv);
+          }
           d1 = fma(yv.x, yv.x, d1); d1 = fma(yv.y, yv.y, d1);
         }
 #pragma unroll
@@ -344,8 +349,14 @@ __global__ void __launch_bounds__(AP_NT) k_apply_generic(const ApplyArgs p) {
         cfma(acc, make_double2(p.beta.x * gl, p.beta.y * gl), tsum);
       }
     }
-    p.y[(size_t)i * ld + a] = acc;
-    if (p.aux) cfma_conj(d0, p.aux[(size_t)i * ld + a], acc);
+    if (p.emode == 2) {
+      const cplx ax = p.aux[(size_t)i * ld + a];
+      acc.x = fma(0.5, ax.x, acc.x); acc.y = fma(0.5, ax.y, acc.y);
+    } else {
+      if (p.emode == 1) { acc = cmul(p.oscale, acc); p.y2[(size_t)i * ld + a] = acc; }
+      p.y[(size_t)i * ld + a] = acc;
+      if (p.aux) cfma_conj(d0, p.aux[(size_t)i * ld + a], acc);
+    }
     d1 = fma(acc.x, acc.x, d1); d1 = fma(acc.y, acc.y, d1);
   }
   if (p.red.fin != FIN_NONE) grid_reduce_finalize<AP_NT>(d0.x, d0.y, d1, p.red);

@@ -21,10 +21,11 @@ static const cplx* blk_ptr(const tdde_handle* h, int blk) {
 }
 
 int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int blk, cplx beta, bool with_terms,
-                  const double* g_dev, const int* step_ptr, int guard, int fin, SolverState* st, const cplx* addv) {
+                  const double* g_dev, const int* step_ptr, int guard, int fin, SolverState* st, const cplx* addv, int emode, cplx oscale, cplx* y2) {
   ApplyArgs a;
   std::memset(&a, 0, sizeof(a));
   a.x = x; a.y = y; a.aux = aux;
+  a.emode = emode; a.oscale = oscale; a.y2 = y2;
   a.addv = (h->path == 1 && with_terms && h->cfg.n_terms > 0) ? addv : nullptr;
   a.n_ang = h->cfg.n_ang; a.n_rad = h->cfg.n_rad; a.ld = h->ld;
   a.seg_len = (with_terms && h->cfg.n_terms > 0) ? h->seg_len : h->seg_len_s;
@@ -91,15 +92,19 @@ int sync_state(tdde_handle* h) {
 }
 
 // The two start-of-step applies and the initial residual (SURVEY 8(a) a2 + a3): with x0 = c,
-//   b = S c - i tau H c,   r0 = b - (S c + i tau H c) = -i dt H c,
-// so one H-apply (t buffer) and one S-apply (s buffer) give both; b itself is only needed through ||b||.
+//   b = S c - i tau H c,   r0 = b - (S c + i tau H c) = -i dt H c,   hence b = S c + r0 / 2,
+// so one H-apply (writing r0 and rhat) and one S-apply (accumulating ||b||^2, storing nothing) give everything.
 static int enqueue_step_start(tdde_handle* h) {
   SolverState* st = h->d_st;
   const cplx one = make_double2(1.0, 0.0);
   int rc;
-  if ((rc = enqueue_apply(h, h->X, h->t, nullptr, BLK_H0, one, true, h->d_g, &st->step_idx, 2, FIN_NONE, st))) return rc;
-  if ((rc = enqueue_apply(h, h->X, h->s, nullptr, BLK_S, one, false, h->d_zero_g, nullptr, 2, FIN_NONE, st))) return rc;
-  h->launches += launch_vec_r0(make_vec_args(h, st, FIN_R0), h->stream);
+  // r0 = rhat = -i dt H c and ||r0||^2, written by the H-apply itself
+  if ((rc = enqueue_apply(h, h->X, h->r, nullptr, BLK_H0, one, true, h->d_g, &st->step_idx, 2, FIN_RES0, st, nullptr, 1,
+                          make_double2(0.0, -h->cfg.dt), h->rhat)))
+    return rc;
+  // ||b||^2 = ||S c + r0 / 2||^2 accumulated by the S-apply, which stores nothing; then the start-of-solve scalars
+  if ((rc = enqueue_apply(h, h->X, h->s, h->r, BLK_S, one, false, h->d_zero_g, nullptr, 2, FIN_R0S, st, nullptr, 2)))
+    return rc;
   return 0;
 }
 

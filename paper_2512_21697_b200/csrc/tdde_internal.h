@@ -68,7 +68,9 @@ enum FinCode {
   FIN_NORM,    // norm_out = Re d0
   FIN_R0,      // d0.x = ||b||^2, d1 = ||r0||^2 -> rho, init, zero-iteration exit
   FIN_S,       // d1 = ||s||^2 -> half-step exit test
-  FIN_R        // d0 = <rhat, r>, d1 = ||r||^2 -> convergence test, rho, beta
+  FIN_R,       // d0 = <rhat, r>, d1 = ||r||^2 -> convergence test, rho, beta
+  FIN_RES0,    // d1 = ||r0||^2 (start of step, from the H-apply that writes r0 and rhat): res2 = d1
+  FIN_R0S      // d1 = ||b||^2 (start of step, from the S-apply): the FIN_R0 logic with ||r0||^2 taken from res2
 };
 
 struct ReduceCtx {
@@ -83,6 +85,10 @@ struct ApplyArgs {
   const cplx* x;           // internal layout
   cplx* y;
   const cplx* aux;         // vector for the fused dot (nullable)
+  int emode;               // write-out: 0 y = result; 1 y = y2 = oscale * result (r0 and rhat); 2 nothing stored,
+                           //   d1 accumulates |result + aux / 2|^2 (||b||^2 with aux = r0, R6)
+  cplx oscale;
+  cplx* y2;
   const cplx* addv;        // banded path, nullable: y = addv + (coupling terms only) x; the block part is skipped
   int n_ang, n_rad, ld;
   int seg_len;             // radial rows per thread
@@ -142,7 +148,6 @@ int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, int
 bool apply_banded_available(int T, int m0, int mstep, int W);
 int launch_apply_generic(const ApplyArgs& a, cudaStream_t s);
 int launch_precond(const PrecArgs& a, cudaStream_t s);
-int launch_vec_r0(const VecArgs& a, cudaStream_t s);
 int launch_vec_p(const VecArgs& a, cudaStream_t s);
 int launch_vec_s(const VecArgs& a, cudaStream_t s);
 int launch_vec_halfexit(const VecArgs& a, cudaStream_t s);

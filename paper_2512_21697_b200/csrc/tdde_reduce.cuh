@@ -46,6 +46,11 @@ __device__ inline void finalize_scalars(SolverState* st, int fin, double d0x, do
   switch (fin) {
     case FIN_NB: st->nb2 = d1; break;
     case FIN_NORM: st->norm_out = d0x; break;
+    case FIN_RES0: st->res2 = d1; break;
+    case FIN_R0S:
+      d0x = d1;                                  // ||b||^2 from this kernel, ||r0||^2 from the previous one
+      d1 = st->res2;
+      // fall through
     case FIN_R0: {
       st->nb2 = d0x;                             // ||b||^2 rides in the first slot
       st->done = 0;

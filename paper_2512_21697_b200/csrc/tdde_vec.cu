@@ -1,4 +1,4 @@
-// tdde_vec.cu -- fused BiCGSTAB vector kernels, layout transposes, small helpers.
+// tdde_vec.cu -- fused BiCGSTAB vector kernels (a3 is fused into the start-of-step applies), layout transposes, small helpers.
 //
 // All of these are HBM-bound streaming kernels: 128-bit (double2) coalesced loads/stores, grid-stride over
 // the internal element count, grid = a fixed multiple of the 148 SMs, the inner products fused into the pass
@@ -16,23 +16,6 @@ static int vec_grid(long long n) {
 }
 
 __device__ __forceinline__ cplx ldcs(const cplx* p) { return __ldcs(p); }
-
-// r = -i dt u (u = H c), rhat = r; nb2 = ||b - i dt/2 u||^2 with b = S c; d1 = ||r||^2       (a3)
-__global__ void __launch_bounds__(VEC_NT) k_vec_r0(VecArgs a) {
-  const SolverState* st = a.red.st;
-  if (st->stalled | (st->status != 0)) return;
-  double nb2 = 0, r2 = 0;
-  const double dt = a.dt, tau = 0.5 * a.dt;
-  for (long long i = (long long)blockIdx.x * VEC_NT + threadIdx.x; i < a.n; i += (long long)gridDim.x * VEC_NT) {
-    cplx u = a.u[i], sc = a.b[i];
-    cplx r = make_double2(dt * u.y, -dt * u.x);          // -i dt u
-    cplx b = make_double2(sc.x + tau * u.y, sc.y - tau * u.x);
-    a.r[i] = r; a.rhat[i] = r;
-    nb2 = fma(b.x, b.x, nb2); nb2 = fma(b.y, b.y, nb2);
-    r2 = fma(r.x, r.x, r2); r2 = fma(r.y, r.y, r2);
-  }
-  grid_reduce_finalize<VEC_NT>(nb2, 0.0, r2, a.red);
-}
 
 // p = r + beta (p - omega v);  first iteration: p = r                                         (a6 i)
 __global__ void __launch_bounds__(VEC_NT) k_vec_p(VecArgs a) {
@@ -190,7 +173,6 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters) {
   if (s == 123.456) out[0] = s;
 }
 
-int launch_vec_r0(const VecArgs& a, cudaStream_t s) { k_vec_r0<<<vec_grid(a.n), VEC_NT, 0, s>>>(a); return 1; }
 int launch_vec_p(const VecArgs& a, cudaStream_t s) { k_vec_p<<<vec_grid(a.n), VEC_NT, 0, s>>>(a); return 1; }
 int launch_vec_s(const VecArgs& a, cudaStream_t s) { k_vec_s<<<vec_grid(a.n), VEC_NT, 0, s>>>(a); return 1; }
 int launch_vec_halfexit(const VecArgs& a, cudaStream_t s) { k_vec_halfexit<<<vec_grid(a.n), VEC_NT, 0, s>>>(a); return 1; }
