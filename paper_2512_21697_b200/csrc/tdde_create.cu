@@ -194,9 +194,11 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     std::vector<zc> Sx(h->blk_count), Hx(h->blk_count), Mx(h->blk_count);
     std::vector<zc> Lc((size_t)c.n_cls * n_rad * w0), Uc((size_t)c.n_cls * n_rad * (w0 + 1));
     // partition count of the preconditioner solve: as many one-warp CTAs as are resident at once (shared memory of
-    // k_precond: 3 stages x 8 rows x TDDE_PC_MAXC (w0+1) complex), never a nearly empty second wave
-    const size_t pc_smem = (size_t)3 * 8 * (TDDE_PC_MAXC * (w0 + 1)) * 16 + 1024;
-    const int pc_slots = 148 * (int)std::min<size_t>(32, (227 * 1024) / pc_smem);
+    // k_precond: 2 stages x 8 rows x TDDE_PC_MAXC (w0+1) complex, and its registers), never a nearly empty second wave
+    const size_t pc_smem = (size_t)2 * 8 * (TDDE_PC_MAXC * (w0 + 1)) * 16 + 1024;
+    const int pc_regs = w0 <= 3 ? 128 : w0 <= 6 ? 144 : w0 <= 9 ? 168 : 208;       // ptxas -v of k_precond<W>
+    const int pc_per_sm = (int)std::min<size_t>(std::min<size_t>(32, (227 * 1024) / pc_smem), 65536 / (pc_regs * 32));
+    const int pc_slots = 148 * pc_per_sm;
     int P = std::max(1, pc_slots / (h->ld / 32));
     if (const char* env = std::getenv("TDDE_PC_PARTS")) P = std::atoi(env);
     const bool templated_w = (w0 == 3 || w0 == 6 || w0 == 9 || w0 == 13);

@@ -16,7 +16,7 @@
 
 #define PC_NT 32
 #define PC_ROWS 8
-#define PC_STAGES 3
+#define PC_STAGES 2
 #define PC_MAXC TDDE_PC_MAXC
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
