@@ -30,7 +30,7 @@ UNIT = "steps/s"
 NUM_SMS = 148
 # dram__bytes_read.sum + dram__bytes_write.sum of one operator-apply launch, from one `ncu --set full` capture
 # (profiles/r01_apply_hbm_ncu.txt); bench.py cannot run ncu itself, so other configs report null
-MEASURED_DRAM_BYTES_PER_APPLY = {"hbm": 1.654e9}
+MEASURED_DRAM_BYTES_PER_APPLY = {"hbm": 2.062e9}
 FP64_FMA_PER_CLK_PER_SM = 64          # B200: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2 TFLOP/s nominal
 
 
