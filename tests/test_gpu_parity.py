@@ -377,3 +377,25 @@ def test_breakdown_is_reported_for_non_finite_input(tiny):
     c = prop.to_device(p.c0)                      # the handle recovers on the next call
     st = prop.propagate(c, p.g_table(2))
     assert st["steps"] == 2 and st["status"] == 0
+
+
+def test_side_stream_and_two_handles(tiny_stress):
+    """A handle bound to a non-default torch stream (the step graph is replayed on the caller's stream) and two live
+    handles used alternately must reproduce the default-stream result bit for bit."""
+    import torch
+    from paper_2512_21697_b200 import Tdde
+    p, prop, _, _ = tiny_stress
+    ref = prop.to_device(p.c0)
+    prop.propagate(ref, p.g_table(8))
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        other = Tdde(p, stream=side)
+        c = other.to_device(p.c0)
+        side.synchronize()
+        for k in range(4):                       # alternate with the default-stream handle, 2 steps at a time
+            other.propagate(c, p.g_table(2, first_step=2 * k))
+            d = prop.to_device(p.c0)
+            prop.propagate(d, p.g_table(1))
+        side.synchronize()
+    assert np.array_equal(c.cpu().numpy(), ref.cpu().numpy())
+    other.close()
