@@ -226,7 +226,7 @@ __device__ __forceinline__ void apply_group(const ApplyArgs& p, const ApplyCommo
 }
 
 template <int T, int M0, int MS, int W, int NG, bool BLK>
-__global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB)) k_apply_banded(const ApplyArgs p) {
+__global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB)) k_apply_banded(const __grid_constant__ ApplyArgs p) {
   using PL = ApplyPlan<T, M0, MS, W, NG, BLK>;
   constexpr int AP_BT = NG * AP_NC;
   constexpr int ND = PL::ND, MAXM = PL::MAXM, XW = PL::XW, JC = PL::JC;
@@ -280,7 +280,8 @@ __global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB
     const int j = jlo + c * JC;
     const int nr = min(JC, jhi - j);
     if (nr <= 0) return;                                     // a chunk of virtual rows only
-    uint32_t bytes = (uint32_t)nr * x_bytes;
+    const bool x2d = (T == 0) && p.use_xmap;                  // one tensor copy: full box, out-of-bounds zero-filled
+    uint32_t bytes = x2d ? (uint32_t)(JC * AP_NC * sizeof(cplx)) : (uint32_t)nr * x_bytes;
     int ncls = 0;
     if (BLK) {
 #pragma unroll
@@ -296,8 +297,15 @@ __global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB
       if (kk >= 0)
         bulk_g2s(st + PL::RS + (size_t)q * JC * ND, p.blk + ((size_t)kk * n_rad + j) * ND, (uint32_t)nr * ND * sizeof(cplx), bar);
     }
-    for (int r = 0; r < nr; ++r)
-      bulk_g2s(st + PL::RS + PL::BS + (size_t)r * XW + x_dst_off, p.x + (size_t)(j + r) * ld + xa_lo, x_bytes, bar);
+    if (x2d) {
+      asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+                       smem_u32(st + PL::RS + PL::BS)),
+                   "l"(reinterpret_cast<uint64_t>(&p.xmap)), "r"(2 * a0), "r"(j), "r"(smem_u32(bar))
+                   : "memory");
+    } else {
+      for (int r = 0; r < nr; ++r)
+        bulk_g2s(st + PL::RS + PL::BS + (size_t)r * XW + x_dst_off, p.x + (size_t)(j + r) * ld + xa_lo, x_bytes, bar);
+    }
   };
   if (threadIdx.x == 0) {
     issue(0);

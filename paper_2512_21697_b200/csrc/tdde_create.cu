@@ -325,6 +325,33 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     CU(cudaMalloc((void**)v, (size_t)h->nint * sizeof(cplx)));
     CU(cudaMemsetAsync(*v, 0, (size_t)h->nint * sizeof(cplx), s));
   }
+  // 2-D tensor maps of the work vectors ([n_rad][2 ld] doubles, box = 128 channels x TDDE_AP_JC rows): the S-only
+  // apply fetches its x tile with one tensor TMA copy per stage instead of one bulk copy per row.  Optional: if the
+  // driver entry point or the encoding is unavailable the kernel keeps using 1-D bulk copies.
+  h->have_xmaps = false;
+  if (h->path == 1 && h->ld >= 128) {
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) == cudaSuccess && fn &&
+        qres == cudaDriverEntryPointSuccess) {
+      bool ok = true;
+      int q = 0;
+      for (cplx** v : vecs) {
+        const cuuint64_t gdim[2] = {(cuuint64_t)2 * h->ld, (cuuint64_t)n_rad};
+        const cuuint64_t gstride[1] = {(cuuint64_t)h->ld * sizeof(cplx)};
+        const cuuint32_t box[2] = {256, TDDE_AP_JC};
+        const cuuint32_t estr[2] = {1, 1};
+        ok = ok && ((encode_fn)fn)(&h->xmaps[q++], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, *v, gdim, gstride, box, estr,
+                                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+      }
+      h->have_xmaps = ok && !std::getenv("TDDE_NO_XMAP");
+    }
+    cudaGetLastError();
+  }
   // state and scratch
   CU(cudaMalloc((void**)&h->d_st, sizeof(SolverState)));
   CU(cudaMalloc((void**)&h->d_st_bench, sizeof(SolverState)));

@@ -37,6 +37,11 @@ int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int b
   a.red.partials = h->d_partials; a.red.ticket = h->d_ticket; a.red.st = st; a.red.fin = fin;
   const int T = with_terms ? h->cfg.n_terms : 0;
   a.n_terms = T;
+  if (T == 0 && h->have_xmaps) {
+    const cplx* vv[9] = {h->X, h->r, h->rhat, h->p, h->v, h->s, h->t, h->y, h->z};
+    for (int q = 0; q < 9; ++q)
+      if (vv[q] == x) { a.xmap = h->xmaps[q]; a.use_xmap = 1; }
+  }
   int rc;
   const bool banded = (h->path == 1);
   if (banded) {

@@ -44,6 +44,8 @@ struct tdde_handle {
   // work vectors (internal layout)
   cplx *X = nullptr, *r = nullptr, *rhat = nullptr, *p = nullptr, *v = nullptr, *s = nullptr, *t = nullptr,
        *y = nullptr, *z = nullptr;
+  CUtensorMap xmaps[9];                      // per work vector (X, r, rhat, p, v, s, t, y, z), for the S-only apply
+  bool have_xmaps = false;
   cplx* c_stage = nullptr;                   // boundary-layout device buffer for tdde_propagate_host
 
   // solver state, scratch

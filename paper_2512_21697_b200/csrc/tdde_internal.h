@@ -6,6 +6,7 @@
 // and the vector accesses are coalesced 16-byte loads.  Pad channels (a >= n_ang) hold zeros throughout.
 // The boundary layout (tdde.h) is channel-major; transposes happen at entry/exit of the API calls.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include "tdde.h"
@@ -82,6 +83,8 @@ struct ReduceCtx {
 
 // ---- operator apply ----
 struct ApplyArgs {
+  CUtensorMap xmap;        // 2-D tensor map of x ([n_rad][2 ld] doubles, box 256 x TDDE_AP_JC), valid iff use_xmap
+  int use_xmap;            // T == 0 kernel only: fetch the x tile of a stage with one tensor TMA copy
   const cplx* x;           // internal layout
   cplx* y;
   const cplx* aux;         // vector for the fused dot (nullable)
