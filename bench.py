@@ -131,7 +131,7 @@ def reference_main(args):
     cb, p = run_oracle(args.config, steps, min(args.warmup, 1), args.sample_ang)
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / cb["value"], "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "complex128 (f64)", "data": "synthetic",
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.config, "note": "CPU oracle on a bounded sample, scaled to the full workload"},
             "cpu_baseline": {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")},
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -244,7 +244,7 @@ def ours_main(args):
         line = {
             "metric": METRIC, "value": steps_per_s, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "complex128 (f64)", "data": "synthetic",
+            "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.config, "n_ang": p.n_ang, "n_rad": p.n_rad, "n": n, "bandwidth": 2 * p.w0 + 1,
                        "n_terms": T, "dt": p.dt, "rtol": p.rtol, "seed": p.seed, "phase": args.phase,
                        "apply_path": prop.apply_path, "parallelism": "replicas only" if world > 1 else "1 GPU",
