@@ -243,7 +243,9 @@ __global__ void __launch_bounds__(128) k_precond_schur_mul(const PrecArgs p) {
 // CTA = 128 channels x PCC_ROWS interior rows.  The spike rows of the CTA's kappa-classes (same class list as the
 // operator apply) are staged in shared memory with cp.async and read back as warp-broadcasts; each thread first
 // issues all of its vector loads, so enough bytes are in flight to stream at HBM speed.
-#define PCC_ROWS 16
+#ifndef PCC_ROWS
+#define PCC_ROWS 8
+#endif
 template <int W>
 __global__ void __launch_bounds__(128) k_precond_correct(const PrecArgs p) {
   if (p.st && solver_idle(p.st)) return;
