@@ -399,3 +399,29 @@ def test_side_stream_and_two_handles(tiny_stress):
         side.synchronize()
     assert np.array_equal(c.cpu().numpy(), ref.cpu().numpy())
     other.close()
+
+
+def test_step_vs_dense_lu_p1_on_gpu(tiny_stress):
+    """P1 on the CUDA path without the oracle: the CN step is the exact solution of the dense system
+    (S + i tau H) c1 = (S - i tau H) c0 built with numpy.kron from the boundary-format inputs."""
+    p, prop, _, _ = tiny_stress
+    n_ang, n_rad = p.n_ang, p.n_rad
+    S = np.zeros((p.n, p.n), dtype=np.complex128)
+    H = np.zeros_like(S)
+    for a in range(n_ang):
+        k = p.cls_of_chan[a]
+        sl = slice(a * n_rad, (a + 1) * n_rad)
+        S[sl, sl] = tdde_inputs.band_to_dense(p.S_band[k])
+        H[sl, sl] = tdde_inputs.band_to_dense(p.H0_band[k])
+    g = p.g_mid(0)
+    for L, t in enumerate(p.terms):
+        A = np.zeros((n_ang, n_ang), dtype=np.complex128)
+        for a in range(n_ang):
+            for q in range(t.A_rowptr[a], t.A_rowptr[a + 1]):
+                A[a, t.A_col[q]] += t.A_val[q]
+        H += g[L] * np.kron(A, tdde_inputs.band_to_dense(t.R_band))
+    tau = 0.5 * p.dt
+    c1 = np.linalg.solve(S + 1j * tau * H, (S - 1j * tau * H) @ p.c0)
+    c = prop.to_device(p.c0)
+    prop.step(c, g)
+    assert rel(c.cpu().numpy(), c1) <= 1e-10
