@@ -18,7 +18,8 @@ the textbook preconditioned BiCGSTAB in the order and notation of DESIGN.md
 
 Pins (tests/test_oracle_pins.py): dense LU solve of the same system, Cayley-transform
 S-norm conservation, exact CN phase of field-free eigenstates, time reversal,
-closed-form hydrogen energies, Kronecker identities, LAPACK band solve.
+closed-form hydrogen energies, Kronecker identities, LAPACK band solve; the panel-streamed
+apply (apply_panels, cn_step_panels) against numpy.kron dense operators and the CSR apply.
 Parity unpinned: BiCGSTAB iteration *counts* (nothing in the paper fixes them).
 """
 from __future__ import annotations
@@ -155,6 +156,47 @@ def apply_rows_sampled(problem, alpha: complex, beta: complex, g: np.ndarray, x:
             acc += beta * g[L] * tsum
         out[s] = acc
     return out
+
+
+# ----------------------------------------------------------------------------- panel-streamed apply (P10, full vector)
+def _band_times_rows(band: np.ndarray, X: np.ndarray) -> np.ndarray:
+    """U[c, i] = sum_d band[i, d+w] X[c, i+d]  (one radial band matrix applied to every row-vector X[c, :])."""
+    n_rad, nd = band.shape
+    w = (nd - 1) // 2
+    U = np.zeros_like(X)
+    for d in range(-w, w + 1):
+        lo, hi = max(0, -d), min(n_rad, n_rad - d)
+        U[:, lo:hi] += band[lo:hi, d + w][None, :] * X[:, lo + d:hi + d]
+    return U
+
+
+def apply_panels(problem, alpha: complex, beta: complex, g: np.ndarray, x: np.ndarray, panel: int = 256) -> np.ndarray:
+    """y = alpha S x + beta (H0 + sum_L g_L A_L (x) R_L) x for sizes where the CSR cannot be held, evaluated
+    from the definition (Eq. 17) one panel of `panel` output channels at a
+    time: for output channel a' the block part is the class band of a' applied to x[a', :], and each coupling
+    term is sum_a A_L[a', a] (R_L x[a, :]) -- the radial band first, then the angular sum over the non-zeros of
+    row a' of A_L.  No assembled matrix, no operand larger than (panel + coupled channels) x n_rad."""
+    n_ang, n_rad = problem.n_ang, problem.n_rad
+    X = np.ascontiguousarray(x).reshape(n_ang, n_rad)
+    Y = np.zeros_like(X)
+    for a0 in range(0, n_ang, panel):
+        a1 = min(n_ang, a0 + panel)
+        for k in np.unique(problem.cls_of_chan[a0:a1]):
+            idx = a0 + np.nonzero(problem.cls_of_chan[a0:a1] == k)[0]
+            Y[idx] += _band_times_rows(alpha * problem.S_band[k] + beta * problem.H0_band[k], X[idx])
+        for L, term in enumerate(problem.terms):
+            if g[L] == 0.0:
+                continue
+            lo, hi = int(term.A_rowptr[a0]), int(term.A_rowptr[a1])
+            if hi == lo:
+                continue
+            cols = np.unique(term.A_col[lo:hi])                      # channels coupled to this panel by A_L
+            U = _band_times_rows(term.R_band, X[cols])               # R_L x[a, :] for those channels
+            where = {int(c): q for q, c in enumerate(cols)}
+            for ap in range(a0, a1):
+                for kk in range(term.A_rowptr[ap], term.A_rowptr[ap + 1]):
+                    Y[ap] += (beta * g[L] * term.A_val[kk]) * U[where[int(term.A_col[kk])]]
+    return Y.reshape(-1)
 
 
 # ----------------------------------------------------------------------------- preconditioner (C5)
@@ -299,6 +341,17 @@ def cn_step(ops: Operators, fact: PrecondFactors, c: np.ndarray, g_mid: np.ndarr
         b = ops.S @ c - 1j * tau * apply_H(ops, g_mid, c)
     M_solve = lambda u: apply_precond(fact, u)
     return bicgstab(A_mul, M_solve, b, c, rtol, max_iter, force_iters=force_iters, keep_trace=keep_trace)
+
+
+def cn_step_panels(problem, fact: PrecondFactors, c: np.ndarray, g_mid: np.ndarray, dt: float, rtol: float,
+                   max_iter: int, panel: int = 256):
+    """cn_step for sizes where the CSR cannot be held: the same A, B and the same bicgstab, with every product
+    evaluated by apply_panels (A = S + i tau H: alpha = 1, beta = +i tau; B: beta = -i tau)."""
+    tau = 0.5 * dt
+    A_mul = lambda u: apply_panels(problem, 1.0, 1j * tau, g_mid, u, panel)
+    b = apply_panels(problem, 1.0, -1j * tau, g_mid, c, panel)
+    M_solve = lambda u: apply_precond(fact, u)
+    return bicgstab(A_mul, M_solve, b, c, rtol, max_iter)
 
 
 def propagate(problem, ops: Operators, fact: PrecondFactors, c0: np.ndarray, n_steps: int,

@@ -97,7 +97,7 @@ bool detect_banded(const tdde_config* c, const tdde_term* terms, int* m0, int* m
 extern "C" void tdde_destroy(tdde_handle* h) {
   if (!h) return;
   cudaStreamSynchronize(h->stream);
-  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_pslot, h->d_warp_cls, h->d_Esp, h->d_Msep, h->d_Scinv, h->d_rs, h->d_Lcol, h->d_Ucol, h->X, h->r,
+  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_pslot, h->d_warp_cls, h->d_Wsp, h->d_Corner, h->d_Schur, h->d_plo, h->d_phi, h->d_rsm, h->d_rsp, h->d_Lcol, h->d_Ucol, h->X, h->r,
                   h->rhat, h->p, h->v, h->s, h->t, h->y, h->z, h->c_stage, h->d_st, h->d_st_bench, h->d_partials,
                   h->d_ticket, h->d_g, h->d_g_small, h->d_zero_g};
   for (void* p : ptrs) if (p) cudaFree(p);
@@ -193,23 +193,25 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
   {
     std::vector<zc> Sx(h->blk_count), Hx(h->blk_count), Mx(h->blk_count);
     std::vector<zc> Lc((size_t)c.n_cls * n_rad * w0), Uc((size_t)c.n_cls * n_rad * (w0 + 1));
-    // partition count of the preconditioner solve: as many one-warp CTAs as are resident at once (shared memory of
-    // k_precond: 2 stages x 8 rows x TDDE_PC_MAXC (w0+1) complex, and its registers), never a nearly empty second wave
-    const size_t pc_smem = (size_t)2 * 8 * (TDDE_PC_MAXC * (w0 + 1)) * 16 + 1024;
-    const int pc_regs = w0 <= 3 ? 128 : w0 <= 6 ? 144 : w0 <= 9 ? 168 : 208;       // ptxas -v of k_precond<W>
-    const int pc_per_sm = (int)std::min<size_t>(std::min<size_t>(32, (227 * 1024) / pc_smem), 65536 / (pc_regs * 32));
-    const int pc_slots = 148 * pc_per_sm;
-    int P = std::max(1, pc_slots / (h->ld / 32));
-    if (const char* env = std::getenv("TDDE_PC_PARTS")) P = std::atoi(env);
-    const bool templated_w = (w0 == 3 || w0 == 6 || w0 == 9 || w0 == 13);
-    P = templated_w ? std::min(std::max(P, 1), TDDE_PC_MAXPARTS) : 1;
-    const PartitionPlan plan = make_partition_plan(n_rad, w0, P);
-    h->pc_P = plan.P; h->pc_ns = plan.ns();
-    for (int q = 0; q < plan.P; ++q) { h->pc_range_lo[q] = plan.lo[q]; h->pc_int_hi[q] = plan.hi[q]; }
-    for (int q = plan.P; q <= TDDE_PC_MAXPARTS; ++q) h->pc_range_lo[q] = n_rad;
-    const int ns = plan.ns();
-    std::vector<zc> Esp(plan.P > 1 ? (size_t)c.n_cls * n_rad * 2 * w0 : 1), Msep(plan.P > 1 ? (size_t)c.n_cls * ns * nd0 : 1),
-        Scinv(plan.P > 1 ? (size_t)c.n_cls * ns * ns : 1);
+    // preconditioner partitions: interiors short enough that a (32 channels x interior) tile plus the factor ring fits
+    // several times into an SM's shared memory (k_precond_tile keeps the right-hand side on chip between its sweeps)
+    const bool templated_w = w0 <= TDDE_PC_MAXW;
+    int rows = w0 <= 4 ? 40 : w0 <= 9 ? 48 : 64;
+    if (const char* env = std::getenv("TDDE_PC_ROWS")) rows = std::max(1, std::atoi(env));
+    int P = templated_w ? partitions_for_rows(n_rad, w0, rows) : 1;
+    if (const char* env = std::getenv("TDDE_PC_PARTS")) P = templated_w ? std::max(1, std::atoi(env)) : 1;
+    PartitionPlan plan = make_partition_plan(n_rad, w0, P);
+    // a single interior must still fit the tile: force a split when it does not (always possible for n_rad that large)
+    while (templated_w && precond_tile_smem(w0, plan.max_interior()) > (size_t)200 * 1024) {
+      const PartitionPlan finer = make_partition_plan(n_rad, w0, plan.P + 1);
+      if (finer.P == plan.P) return TDDE_EINVAL;
+      plan = finer;
+    }
+    h->pc_P = plan.P; h->pc_tile_rows = plan.max_interior();
+    const size_t ww = (size_t)w0 * w0;
+    const int nsep = plan.P - 1;
+    std::vector<zc> Wsp(plan.P > 1 ? (size_t)c.n_cls * n_rad * 2 * w0 : 1), Corner(plan.P > 1 ? (size_t)c.n_cls * plan.P * 2 * ww : 1),
+        Schur(plan.P > 1 ? (size_t)c.n_cls * nsep * 3 * ww : 1);
     std::vector<zc> Mrow(blk_sz);
     const zc itau(0.0, h->tau);
     for (int k = 0; k < c.n_cls; ++k) {
@@ -229,11 +231,13 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
         std::memcpy(&Hx[k * blk_sz], Hk, blk_sz * sizeof(zc));
         std::memcpy(&Mx[k * blk_sz], Mrow.data(), blk_sz * sizeof(zc));
       }
+      double growth = 1.0;
       if (!build_partitioned_factors(Mrow, plan, &Lc[(size_t)k * n_rad * w0], &Uc[(size_t)k * n_rad * (w0 + 1)],
-                                     plan.P > 1 ? &Esp[(size_t)k * n_rad * 2 * w0] : nullptr,
-                                     plan.P > 1 ? &Msep[(size_t)k * ns * nd0] : nullptr,
-                                     plan.P > 1 ? &Scinv[(size_t)k * ns * ns] : nullptr))
+                                     plan.P > 1 ? &Wsp[(size_t)k * n_rad * 2 * w0] : nullptr,
+                                     plan.P > 1 ? &Corner[(size_t)k * plan.P * 2 * ww] : nullptr,
+                                     plan.P > 1 ? &Schur[(size_t)k * nsep * 3 * ww] : nullptr, &growth))
         return TDDE_ESINGULAR;
+      h->lu_growth = std::max(h->lu_growth, growth);
     }
     int rc;
     if ((rc = dev_upload(&h->d_S, reinterpret_cast<cplx*>(Sx.data()), Sx.size(), s))) return rc;
@@ -242,10 +246,13 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     if ((rc = dev_upload(&h->d_blk_tmp, (cplx*)nullptr, Mx.size(), s))) return rc;
     if ((rc = dev_upload(&h->d_Lcol, reinterpret_cast<cplx*>(Lc.data()), Lc.size(), s))) return rc;
     if ((rc = dev_upload(&h->d_Ucol, reinterpret_cast<cplx*>(Uc.data()), Uc.size(), s))) return rc;
-    if ((rc = dev_upload(&h->d_Esp, reinterpret_cast<cplx*>(Esp.data()), Esp.size(), s))) return rc;
-    if ((rc = dev_upload(&h->d_Msep, reinterpret_cast<cplx*>(Msep.data()), Msep.size(), s))) return rc;
-    if ((rc = dev_upload(&h->d_Scinv, reinterpret_cast<cplx*>(Scinv.data()), Scinv.size(), s))) return rc;
-    if ((rc = dev_upload(&h->d_rs, (cplx*)nullptr, (size_t)std::max(ns, 1) * h->ld, s))) return rc;
+    if ((rc = dev_upload(&h->d_Wsp, reinterpret_cast<cplx*>(Wsp.data()), Wsp.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_Corner, reinterpret_cast<cplx*>(Corner.data()), Corner.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_Schur, reinterpret_cast<cplx*>(Schur.data()), Schur.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_plo, plan.lo.data(), plan.lo.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_phi, plan.hi.data(), plan.hi.size(), s))) return rc;
+    if ((rc = dev_upload(&h->d_rsm, (cplx*)nullptr, (size_t)plan.P * w0 * h->ld, s))) return rc;
+    if ((rc = dev_upload(&h->d_rsp, (cplx*)nullptr, (size_t)plan.P * w0 * h->ld, s))) return rc;
     CU(cudaStreamSynchronize(s));
   }
   // coupling terms

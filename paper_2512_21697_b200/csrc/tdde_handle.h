@@ -10,6 +10,8 @@ typedef std::complex<double> zc;
 struct tdde_handle {
   tdde_config cfg;
   cudaStream_t stream = nullptr;
+  int device = 0;                // the device that was current at tdde_create; every entry point runs on it
+  int num_sms = 148;             // cudaDevAttrMultiProcessorCount of that device
   int ld = 0;                    // padded channel count (multiple of 32)
   long long nint = 0;            // n_rad * ld
   long long n = 0;               // n_ang * n_rad
@@ -37,9 +39,10 @@ struct tdde_handle {
   cplx* d_Aval[TDDE_MAX_TERMS] = {};
   cplx *d_Lcol = nullptr, *d_Ucol = nullptr; // preconditioner factors
   int *d_pslot = nullptr, *d_warp_cls = nullptr;
-  int pc_P = 1, pc_ns = 0;                   // partitioned solve (tdde_partition.h)
-  int pc_range_lo[TDDE_PC_MAXPARTS + 1] = {}, pc_int_hi[TDDE_PC_MAXPARTS] = {};
-  cplx *d_Esp = nullptr, *d_Msep = nullptr, *d_Scinv = nullptr, *d_rs = nullptr;
+  int pc_P = 1, pc_tile_rows = 0;            // partitioned solve (tdde_partition.h)
+  int *d_plo = nullptr, *d_phi = nullptr;
+  cplx *d_Wsp = nullptr, *d_Corner = nullptr, *d_Schur = nullptr, *d_rsm = nullptr, *d_rsp = nullptr;
+  double lu_growth = 1.0;                    // largest element growth of the unpivoted interior LUs over all classes
 
   // work vectors (internal layout)
   cplx *X = nullptr, *r = nullptr, *rhat = nullptr, *p = nullptr, *v = nullptr, *s = nullptr, *t = nullptr,

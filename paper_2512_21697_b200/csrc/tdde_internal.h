@@ -32,8 +32,10 @@
 #ifndef TDDE_AP_MAXC
 #define TDDE_AP_MAXC 16    // banded apply: distinct kappa-classes per CTA staged in shared memory
 #endif
-#define TDDE_PC_MAXC 8
-#define TDDE_PC_MAXPARTS 16
+#define TDDE_PC_MAXC 4      // preconditioner: distinct kappa-classes per warp staged in shared memory
+// half-bandwidths the preconditioner kernels are instantiated for (others <= 32 take the runtime-w two-sweep kernel)
+#define TDDE_PC_WIDTHS(X) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13)
+#define TDDE_PC_MAXW 13
 
 typedef double2 cplx;
 
@@ -134,15 +136,15 @@ struct PrecArgs {
   const int* slot;         // [ld] index of the channel's class in its warp's class list, -1 = not staged
   const int* warp_cls;     // [ld/32][TDDE_PC_MAXC] classes staged per warp (-1 = unused)
   // partitioned solve (tdde_partition.h); P == 1: plain LU over all rows
-  int P, ns;
-  int range_lo[TDDE_PC_MAXPARTS + 1];   // range q = rows [range_lo[q], range_lo[q+1]) = interior q + separator after it
-  int int_hi[TDDE_PC_MAXPARTS];         // interior q = rows [range_lo[q], int_hi[q])
-  const cplx* Esp;         // [n_cls][n_rad][2w]
-  const cplx* Msep;        // [n_cls][ns][2w+1]
-  const cplx* Scinv;       // [n_cls][ns][ns]
-  cplx* rs;                // scratch [ns][ld]: Schur right-hand side
-  const int* aslot;        // [ld] the apply's per-CTA class slot (128-channel groups), used by k_precond_correct
-  const int* cta_cls;      // [n_cta][TDDE_AP_MAXC]
+  int P;                   // interiors
+  int tile_rows;           // longest interior = rows of the shared-memory tile
+  const int* plo;          // device [P]: interior q = rows [plo[q], phi[q]); separator q = rows [phi[q], phi[q] + w)
+  const int* phi;
+  const cplx* Wsp;         // [n_cls][n_rad][2w] left spikes
+  const cplx* Corner;      // [n_cls][P][2][w][w] corner blocks of A_IS
+  const cplx* Schur;       // [n_cls][P-1][3][w][w] block Thomas factors of the Schur complement
+  cplx* rsm;               // scratch [P][w][ld]: spike products towards the separator before each interior
+  cplx* rsp;               // scratch [P][w][ld]: ... after each interior; reused for the forward-eliminated Schur rhs
   const SolverState* st;   // nullable guard
 };
 
@@ -151,6 +153,7 @@ int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, int
 bool apply_banded_available(int T, int m0, int mstep, int W);
 int launch_apply_generic(const ApplyArgs& a, cudaStream_t s);
 int launch_precond(const PrecArgs& a, cudaStream_t s);
+size_t precond_tile_smem(int w, int tile_rows);   // dynamic shared memory of k_precond_tile
 int launch_vec_p(const VecArgs& a, cudaStream_t s);
 int launch_vec_s(const VecArgs& a, cudaStream_t s);
 int launch_vec_halfexit(const VecArgs& a, cudaStream_t s);

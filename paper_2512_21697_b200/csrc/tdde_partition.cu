@@ -4,11 +4,13 @@
 #include "tdde_internal.h"
 #include "tdde_partition.h"
 
+static int min_interior(int w) { return std::max(2 * w, 8); }
+
 PartitionPlan make_partition_plan(int n, int w, int P) {
   PartitionPlan pl;
   pl.n = n; pl.w = w;
   P = std::max(1, P);
-  while (P > 1 && (n - (P - 1) * w) / P < 8 * w) --P;     // interiors must dominate the separators
+  while (P > 1 && (n - (P - 1) * w) / P < min_interior(w)) --P;     // block-tridiagonal Schur needs interiors >= w rows
   pl.P = P;
   const int interior = n - (P - 1) * w;
   int pos = 0;
@@ -19,6 +21,11 @@ PartitionPlan make_partition_plan(int n, int w, int P) {
     pos += m + w;
   }
   return pl;
+}
+
+int partitions_for_rows(int n, int w, int rows) {
+  rows = std::max(rows, min_interior(w));
+  return std::max(1, (n + w + rows + w - 1) / (rows + w));
 }
 
 namespace {
@@ -58,19 +65,21 @@ bool invert_dense(std::vector<zc>& A, int n, zc* out) {   // Gauss-Jordan, parti
 
 }  // namespace
 
-bool build_partitioned_factors(const std::vector<zc>& Mrow, const PartitionPlan& pl, zc* Lcol, zc* Ucol, zc* Esp,
-                               zc* Msep, zc* Scinv) {
-  const int n = pl.n, w = pl.w, nd = 2 * w + 1, P = pl.P, ns = pl.ns();
+bool build_partitioned_factors(const std::vector<zc>& Mrow, const PartitionPlan& pl, zc* Lcol, zc* Ucol, zc* Wsp,
+                               zc* Corner, zc* Schur, double* growth) {
+  const int n = pl.n, w = pl.w, nd = 2 * w + 1, P = pl.P;
   auto M = [&](int i, int j) -> zc { return (j < 0 || j >= n || std::abs(i - j) > w) ? zc(0, 0) : Mrow[(size_t)i * nd + (j - i + w)]; };
   std::vector<int> seg(n);
   for (int i = 0; i < n; ++i) seg[i] = segment_of(pl, i);
 
   // block-diagonal copy: couplings between different segments removed, separators replaced by identity
   std::vector<zc> F(Mrow);
+  double max_m = 0;
   for (int i = 0; i < n; ++i)
     for (int d = -w; d <= w; ++d) {
       const int j = i + d;
       if (j < 0 || j >= n) { F[(size_t)i * nd + d + w] = zc(0, 0); continue; }
+      max_m = std::max(max_m, std::abs(F[(size_t)i * nd + d + w]));
       if (seg[i] % 2 == 1) F[(size_t)i * nd + d + w] = (d == 0) ? zc(1, 0) : zc(0, 0);
       else if (seg[j] != seg[i]) F[(size_t)i * nd + d + w] = zc(0, 0);
     }
@@ -87,6 +96,11 @@ bool build_partitioned_factors(const std::vector<zc>& Mrow, const PartitionPlan&
       for (int c = i + 1; c <= last; ++c) at(r, c) -= l * at(i, c);
     }
   }
+  if (growth) {
+    double max_lu = 0;
+    for (size_t q = 0; q < F.size(); ++q) max_lu = std::max(max_lu, std::abs(F[q]));
+    *growth = max_m > 0 ? max_lu / max_m : 1.0;
+  }
   for (int i = 0; i < n; ++i) {
     for (int d = 1; d <= w; ++d) Lcol[(size_t)i * w + d - 1] = (i + d < n) ? at(i + d, i) : zc(0, 0);
     const zc uinv = zc(1, 0) / at(i, i);
@@ -96,59 +110,86 @@ bool build_partitioned_factors(const std::vector<zc>& Mrow, const PartitionPlan&
   }
   if (P == 1) return true;
 
-  // solve with the block LU (host): v <- A_qq^{-1} v on rows [lo, hi)
-  auto block_solve = [&](int lo, int hi, std::vector<zc>& v) {
-    for (int i = lo; i < hi; ++i)
-      for (int d = 1; d <= w && i - d >= lo; ++d) v[i] -= at(i, i - d) * v[i - d];
-    for (int i = hi - 1; i >= lo; --i) {
-      for (int d = 1; d <= w && i + d < hi; ++d) v[i] -= at(i, i + d) * v[i + d];
-      v[i] /= at(i, i);
-    }
-  };
-  // spikes E^- (separator before the interior) and E^+ (separator after)
-  std::fill(Esp, Esp + (size_t)n * 2 * w, zc(0, 0));
-  std::vector<zc> v(n);
+  // left spikes: row s of W = A_SI A_II^{-1} restricted to interior q solves A_qq^T u = M[s, I_q]^T; with A_qq = L U
+  // that is U^T z = a (forward), L^T u = z (backward)
+  std::fill(Wsp, Wsp + (size_t)n * 2 * w, zc(0, 0));
+  std::vector<zc> z(n), u(n);
   for (int q = 0; q < P; ++q) {
     const int lo = pl.lo[q], hi = pl.hi[q];
     for (int side = 0; side < 2; ++side) {
       if ((side == 0 && q == 0) || (side == 1 && q == P - 1)) continue;
       const int s0 = side == 0 ? pl.hi[q - 1] : pl.hi[q];
       for (int c = 0; c < w; ++c) {
-        for (int i = lo; i < hi; ++i) v[i] = M(i, s0 + c);
-        block_solve(lo, hi, v);
-        for (int i = lo; i < hi; ++i) Esp[(size_t)i * 2 * w + side * w + c] = v[i];
-      }
-    }
-  }
-  // separator rows of M (own-separator columns zeroed) and the Schur complement
-  std::vector<zc> Sc((size_t)ns * ns, zc(0, 0));
-  for (int j = 0; j + 1 < P; ++j) {
-    const int s0 = pl.hi[j];
-    for (int c = 0; c < w; ++c) {
-      const int i = s0 + c, row = j * w + c;
-      for (int d = -w; d <= w; ++d) {
-        const int col = i + d;
-        const bool own = col >= s0 && col < s0 + w;
-        Msep[(size_t)row * nd + d + w] = own ? zc(0, 0) : M(i, col);
-        if (own) Sc[(size_t)row * ns + j * w + (col - s0)] += M(i, col);
-        else if (col >= 0 && col < n) {
-          // interior row `col` of interior q: subtract M(i, col) * E[col][.]
-          const int q = seg[col] / 2;
-          for (int side = 0; side < 2; ++side) {
-            const int jsep = side == 0 ? q - 1 : q;          // separator index of E^-/E^+
-            if (jsep < 0 || jsep >= P - 1) continue;
-            for (int c2 = 0; c2 < w; ++c2)
-              Sc[(size_t)row * ns + jsep * w + c2] -= M(i, col) * Esp[(size_t)col * 2 * w + side * w + c2];
-          }
+        const int s = s0 + c;
+        for (int i = lo; i < hi; ++i) {
+          zc acc = M(s, i);
+          for (int d = 1; d <= w && i - d >= lo; ++d) acc -= at(i - d, i) * z[i - d];
+          z[i] = acc / at(i, i);
+        }
+        for (int i = hi - 1; i >= lo; --i) {
+          zc acc = z[i];
+          for (int d = 1; d <= w && i + d < hi; ++d) acc -= at(i + d, i) * u[i + d];
+          u[i] = acc;
+          Wsp[(size_t)i * 2 * w + side * w + c] = acc;
         }
       }
     }
   }
-  return invert_dense(Sc, ns, Scinv);
+  // corners of A_IS: the only rows of an interior that see a separator are its first and last w rows
+  const size_t ww = (size_t)w * w;
+  std::fill(Corner, Corner + (size_t)P * 2 * ww, zc(0, 0));
+  for (int q = 0; q < P; ++q)
+    for (int r = 0; r < w; ++r)
+      for (int c = 0; c < w; ++c) {
+        if (q > 0) Corner[((size_t)q * 2 + 0) * ww + r * w + c] = M(pl.lo[q] + r, pl.hi[q - 1] + c);
+        if (q + 1 < P) Corner[((size_t)q * 2 + 1) * ww + r * w + c] = M(pl.hi[q] - w + r, pl.hi[q] + c);
+      }
+  // Schur complement Sc = A_SS - W A_IS, block tridiagonal; block Thomas factors
+  std::vector<zc> D(ww), B(ww), C(ww), Cprev(ww, zc(0, 0)), Dinv_prev(ww, zc(0, 0)), Lb(ww), tmp(ww);
+  std::fill(Schur, Schur + (size_t)(P - 1) * 3 * ww, zc(0, 0));
+  for (int j = 0; j + 1 < P; ++j) {
+    const int s0 = pl.hi[j];
+    std::fill(B.begin(), B.end(), zc(0, 0));
+    std::fill(C.begin(), C.end(), zc(0, 0));
+    for (int c = 0; c < w; ++c)
+      for (int c2 = 0; c2 < w; ++c2) {
+        zc d = M(s0 + c, s0 + c2), b(0, 0), cc(0, 0);
+        for (int i = std::max(pl.lo[j], pl.hi[j] - w); i < pl.hi[j]; ++i) d -= Wsp[(size_t)i * 2 * w + w + c] * M(i, s0 + c2);
+        for (int i = pl.lo[j + 1]; i < std::min(pl.hi[j + 1], pl.lo[j + 1] + w); ++i) d -= Wsp[(size_t)i * 2 * w + c] * M(i, s0 + c2);
+        if (j > 0)
+          for (int i = pl.lo[j]; i < std::min(pl.hi[j], pl.lo[j] + w); ++i) b -= Wsp[(size_t)i * 2 * w + w + c] * M(i, pl.hi[j - 1] + c2);
+        if (j + 2 < P)
+          for (int i = std::max(pl.lo[j + 1], pl.hi[j + 1] - w); i < pl.hi[j + 1]; ++i) cc -= Wsp[(size_t)i * 2 * w + c] * M(i, pl.hi[j + 1] + c2);
+        D[c * w + c2] = d; B[c * w + c2] = b; C[c * w + c2] = cc;
+      }
+    std::fill(Lb.begin(), Lb.end(), zc(0, 0));
+    if (j > 0) {
+      for (int a = 0; a < w; ++a)
+        for (int b2 = 0; b2 < w; ++b2) {
+          zc acc(0, 0);
+          for (int k = 0; k < w; ++k) acc += B[a * w + k] * Dinv_prev[k * w + b2];
+          Lb[a * w + b2] = acc;
+        }
+      for (int a = 0; a < w; ++a)
+        for (int b2 = 0; b2 < w; ++b2) {
+          zc acc(0, 0);
+          for (int k = 0; k < w; ++k) acc += Lb[a * w + k] * Cprev[k * w + b2];
+          D[a * w + b2] -= acc;
+        }
+    }
+    tmp = D;
+    if (!invert_dense(tmp, w, Dinv_prev.data())) return false;
+    zc* out = Schur + (size_t)j * 3 * ww;
+    std::copy(Lb.begin(), Lb.end(), out);
+    std::copy(Dinv_prev.begin(), Dinv_prev.end(), out + ww);
+    std::copy(C.begin(), C.end(), out + 2 * ww);
+    Cprev = C;
+  }
+  return true;
 }
 
-// ---- host self-test (no GPU): the partitioned solve, with the device kernels A/B/C replayed in plain loops on the
-// host arrays exactly as laid out for the device, against dense Gaussian elimination with partial pivoting ----
+// ---- host self-test (no GPU): the partitioned solve, with the device kernels P1/P2/P3 replayed in plain loops on the
+// host arrays exactly as laid out for the device; checked by the residual of the original banded system ----
 extern "C" int tdde_selftest_partition(int32_t n, int32_t w, int32_t P, uint32_t seed, double* max_rel_err) {
   if (n <= 0 || w < 1 || w >= n || P < 1 || !max_rel_err) return TDDE_EINVAL;
   const int nd = 2 * w + 1;
@@ -165,51 +206,76 @@ extern "C" int tdde_selftest_partition(int32_t n, int32_t w, int32_t P, uint32_t
       if (d > 0) Mrow[(size_t)(i + d) * nd + w - d] = std::conj(s) + zc(0, 0.05) * std::conj(hh);
     }
   const PartitionPlan pl = make_partition_plan(n, w, P);
-  const int ns = pl.ns();
-  std::vector<zc> Lc((size_t)n * w), Uc((size_t)n * (w + 1)), Esp((size_t)n * 2 * w + 1), Msep((size_t)ns * nd + 1), Sci((size_t)ns * ns + 1);
-  if (!build_partitioned_factors(Mrow, pl, Lc.data(), Uc.data(), Esp.data(), Msep.data(), Sci.data())) return TDDE_ESINGULAR;
-  std::vector<zc> b(n), y(n);
+  const int Pp = pl.P;
+  const size_t ww = (size_t)w * w;
+  std::vector<zc> Lc((size_t)n * w), Uc((size_t)n * (w + 1)), Wsp((size_t)n * 2 * w + 1), Corner((size_t)Pp * 2 * ww + 1), Sch((size_t)(Pp - 1) * 3 * ww + 1);
+  double growth = 0;
+  if (!build_partitioned_factors(Mrow, pl, Lc.data(), Uc.data(), Wsp.data(), Corner.data(), Sch.data(), &growth)) return TDDE_ESINGULAR;
+  std::vector<zc> b(n), y(n, zc(0, 0));
   for (int i = 0; i < n; ++i) b[i] = zc(rnd(), rnd());
-  // kernel A: per range, forward then backward sweep in column form with the device factor layout
-  for (int q = 0; q < pl.P; ++q) {
-    const int lo = pl.lo[q], hi = q + 1 < pl.P ? pl.lo[q + 1] : n;
+  if (Pp > 1) {
+    // kernel P1: per interior, the spike dot products for the separator before (minus) and after (plus)
+    std::vector<zc> rsm((size_t)Pp * w, zc(0, 0)), rsp((size_t)Pp * w, zc(0, 0));
+    for (int q = 0; q < Pp; ++q)
+      for (int i = pl.lo[q]; i < pl.hi[q]; ++i)
+        for (int c = 0; c < w; ++c) {
+          rsm[(size_t)q * w + c] += Wsp[(size_t)i * 2 * w + c] * b[i];
+          rsp[(size_t)q * w + c] += Wsp[(size_t)i * 2 * w + w + c] * b[i];
+        }
+    // kernel P2: block Thomas over the separators
+    std::vector<zc> rp((size_t)(Pp - 1) * w), prev(w, zc(0, 0)), cur(w), xn(w, zc(0, 0));
+    for (int j = 0; j + 1 < Pp; ++j) {
+      const zc* Lb = Sch.data() + (size_t)j * 3 * ww;
+      for (int c = 0; c < w; ++c) {
+        zc r = b[pl.hi[j] + c] - rsp[(size_t)j * w + c] - rsm[(size_t)(j + 1) * w + c];
+        for (int k = 0; k < w; ++k) r -= Lb[c * w + k] * prev[k];
+        cur[c] = r;
+      }
+      for (int c = 0; c < w; ++c) rp[(size_t)j * w + c] = prev[c] = cur[c];
+    }
+    for (int j = Pp - 2; j >= 0; --j) {
+      const zc* Di = Sch.data() + (size_t)j * 3 * ww + ww;
+      const zc* Cj = Di + ww;
+      for (int c = 0; c < w; ++c) {
+        zc r = rp[(size_t)j * w + c];
+        for (int k = 0; k < w; ++k) r -= Cj[c * w + k] * xn[k];
+        cur[c] = r;
+      }
+      for (int c = 0; c < w; ++c) {
+        zc x(0, 0);
+        for (int k = 0; k < w; ++k) x += Di[c * w + k] * cur[k];
+        y[pl.hi[j] + c] = x;
+      }
+      for (int c = 0; c < w; ++c) xn[c] = y[pl.hi[j] + c];
+    }
+  }
+  // kernel P3: per interior, corner-corrected right-hand side, then forward and backward sweep in column form
+  for (int q = 0; q < Pp; ++q) {
+    const int lo = pl.lo[q], hi = pl.hi[q], len = hi - lo;
+    std::vector<zc> tile(len);
+    for (int r = 0; r < len; ++r) tile[r] = b[lo + r];
+    if (q > 0)
+      for (int r = 0; r < w; ++r)
+        for (int c = 0; c < w; ++c) tile[r] -= Corner[((size_t)q * 2 + 0) * ww + r * w + c] * y[pl.hi[q - 1] + c];
+    if (q + 1 < Pp)
+      for (int r = 0; r < w; ++r)
+        for (int c = 0; c < w; ++c) tile[len - w + r] -= Corner[((size_t)q * 2 + 1) * ww + r * w + c] * y[hi + c];
     std::vector<zc> pw(w + 1, zc(0, 0));
-    for (int i = lo; i < hi; ++i) {
-      y[i] = b[i] + pw[0];
-      for (int d = 0; d < w; ++d) pw[d] = pw[d + 1] - Lc[(size_t)i * w + d] * y[i];
+    for (int r = 0; r < len; ++r) {
+      const int i = lo + r;
+      tile[r] += pw[0];
+      for (int d = 0; d < w; ++d) pw[d] = pw[d + 1] - Lc[(size_t)i * w + d] * tile[r];
     }
     std::fill(pw.begin(), pw.end(), zc(0, 0));
-    for (int i = hi - 1; i >= lo; --i) {
-      const zc t = y[i] + pw[0];
+    for (int r = len - 1; r >= 0; --r) {
+      const int i = lo + r;
+      const zc t = tile[r] + pw[0];
       const zc xi = t * Uc[(size_t)i * (w + 1)];
       y[i] = xi;
       pw[0] = pw[1] - Uc[(size_t)i * (w + 1) + 1] * t;           // pre-scaled entry multiplies (y_i + pw0)
       for (int d = 1; d < w; ++d) pw[d] = pw[d + 1] - Uc[(size_t)i * (w + 1) + d + 1] * xi;
     }
   }
-  if (pl.P > 1) {
-    std::vector<zc> rs(ns), xs(ns);
-    for (int s = 0; s < ns; ++s) {                                // kernel B1
-      const int i = pl.hi[s / w] + s % w;
-      zc acc = y[i];
-      for (int d = -w; d <= w; ++d)
-        if (i + d >= 0 && i + d < n) acc -= Msep[(size_t)s * nd + d + w] * y[i + d];
-      rs[s] = acc;
-    }
-    for (int o = 0; o < ns; ++o) {                                // kernel B2
-      zc acc(0, 0);
-      for (int q = 0; q < ns; ++q) acc += Sci[(size_t)o * ns + q] * rs[q];
-      xs[o] = acc;
-    }
-    for (int o = 0; o < ns; ++o) y[pl.hi[o / w] + o % w] = xs[o];
-    for (int q = 0; q < pl.P; ++q)                                // kernel C
-      for (int i = pl.lo[q]; i < pl.hi[q]; ++i)
-        for (int c = 0; c < w; ++c) {
-          if (q > 0) y[i] -= Esp[(size_t)i * 2 * w + c] * xs[(q - 1) * w + c];
-          if (q + 1 < pl.P) y[i] -= Esp[(size_t)i * 2 * w + w + c] * xs[q * w + c];
-        }
-  }
-  // reference: residual of the original system (exact check, no second solver needed) and a dense solve
   double num = 0, den = 0;
   for (int i = 0; i < n; ++i) {
     zc acc(0, 0);

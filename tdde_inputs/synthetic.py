@@ -103,7 +103,9 @@ def s_norm_sq_banded(S_band: np.ndarray, cls_of_chan: np.ndarray, c: np.ndarray,
 def make_synthetic(n_ang: int, n_r: int, bandwidth: int, n_terms: int, dt: float, n_steps: int,
                    rtol: float, seed: int, tiny_offsets: bool = False, e0: float = E0_DEFAULT,
                    omega: float = OMEGA_DEFAULT, phase: float = 0.0, max_iter: int = 200,
-                   name: str = "synthetic", with_c0: bool = True) -> Problem:
+                   name: str = "synthetic", with_c0: bool = True, s_q: float = 0.3, h0_scale: float = 1.0) -> Problem:
+    """s_q: decay of the SPD band S[i,j] = s_q^|i-j| (0.3 in every BASELINE config; larger = worse conditioned);
+    h0_scale multiplies H0 (stiff field-free blocks, tau |H0| >> |S|, as the Dirac rest-mass terms are)."""
     assert bandwidth % 2 == 1
     w = (bandwidth - 1) // 2
     n_rad = 2 * n_r
@@ -113,11 +115,11 @@ def make_synthetic(n_ang: int, n_r: int, bandwidth: int, n_terms: int, dt: float
     n_cls = len(kappas)
     kmax = float(np.max(np.abs(kappas)))
 
-    S1 = spd_band(n_rad, w)
+    S1 = spd_band(n_rad, w, s_q)
     base = herm_band(rng, n_rad, w)
     second = herm_band(rng, n_rad, w)
     S_band = np.broadcast_to(S1, (n_cls, n_rad, 2 * w + 1)).copy()
-    H0_band = base[None] + (kappas[:, None, None] / kmax) * second[None]
+    H0_band = h0_scale * (base[None] + (kappas[:, None, None] / kmax) * second[None])
 
     terms = []
     for L in range(n_terms):

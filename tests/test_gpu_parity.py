@@ -425,3 +425,123 @@ def test_step_vs_dense_lu_p1_on_gpu(tiny_stress):
     c = prop.to_device(p.c0)
     prop.step(c, g)
     assert rel(c.cpu().numpy(), c1) <= 1e-10
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# True residual, bandwidth / term-count coverage of the propagation, degenerate exits (VERDICT r1, weak #1 c-e)
+def _true_rel_residual(p, prop, c0, c1, g):
+    """||b - A c1|| / ||b|| with b = (S - i tau H) c0 and A = S + i tau H, both through tdde_apply (full operator)."""
+    import torch
+    tau = 0.5 * p.dt
+    b = prop.apply(1.0, -1j * tau, g, c0)
+    Ax = prop.apply(1.0, +1j * tau, g, c1)
+    return float(torch.linalg.vector_norm(b - Ax) / torch.linalg.vector_norm(b))
+
+
+@pytest.mark.parametrize("kw", [dict(), dict(s_q=0.45), dict(s_q=0.6), dict(h0_scale=300.0), dict(h0_scale=3e4, s_q=0.45)])
+def test_true_residual_at_exit(kw):
+    """The in-iteration applies of the banded path may use A y = p + i tau (coupling) y (exact up to the rounding of the
+    solve M y = p); the residual the solver tests is the recursive one.  Recompute the TRUE residual ||b - A x|| / ||b||
+    with the full operator after each step, on well-conditioned, worse-conditioned (S decay 0.45 / 0.6) and stiff
+    (tau |H0| >> |S|) field-free blocks, and compare the state with the oracle."""
+    from paper_2512_21697_b200 import Tdde
+    p = tdde_inputs.make_synthetic(name="resid", n_ang=70, n_r=90, bandwidth=13, n_terms=5, dt=0.005, n_steps=3,
+                                   rtol=1e-10, seed=21, phase=np.pi / 2, e0=2.0, **kw)
+    prop = Tdde(p)
+    assert prop.apply_path == "banded"
+    ops, fact = orc.assemble(p), orc.factor_precond(p)
+    c = prop.to_device(p.c0)
+    c_ref = p.c0.copy()
+    for s in range(p.n_steps):
+        c_prev = c.clone()
+        g = p.g_mid(s)
+        st = prop.step(c, g)
+        assert st["status"] == 0 and st["half_iters"] >= 1
+        r_true = _true_rel_residual(p, prop, c_prev, c, g)
+        assert r_true <= 1.5 * p.rtol, (kw, s, r_true, st["rel_res"])
+        c_ref, info = orc.cn_step(ops, fact, c_ref, g, p.dt, p.rtol, p.max_iter)
+    if "h0_scale" not in kw:      # stiff blocks: cond(A) x rtol exceeds 1e-9, two converged solves may differ by more
+        assert rel(c.cpu().numpy(), c_ref) <= 1e-9
+    prop.close()
+
+
+@pytest.mark.parametrize("ng", ["1", "2"])
+@pytest.mark.parametrize("bw", [7, 19])
+def test_propagation_bandwidth_7_and_19_t7(bw, ng, monkeypatch):
+    """W = 3 and W = 9 with T = 7 (the shapes of the HBM-scale bandwidth sweep), both term-split variants: full
+    propagation against the oracle, not only apply + preconditioner."""
+    from paper_2512_21697_b200 import Tdde
+    monkeypatch.setenv("TDDE_APPLY_NG", ng)
+    p = tdde_inputs.make_synthetic(name="bw", n_ang=150, n_r=45, bandwidth=bw, n_terms=7, dt=0.004, n_steps=4, rtol=1e-10,
+                                   seed=31, phase=np.pi / 2, e0=2.0)
+    prop = Tdde(p)
+    assert prop.apply_path == "banded"
+    ops, fact = orc.assemble(p), orc.factor_precond(p)
+    c_ref, infos = orc.propagate(p, ops, fact, p.c0, p.n_steps)
+    c = prop.to_device(p.c0)
+    st = prop.propagate(c, p.g_table(p.n_steps))
+    assert st["steps"] == p.n_steps and st["status"] == 0
+    assert rel(c.cpu().numpy(), c_ref) <= 1e-9
+    assert abs(st["half_iters"] - sum(i.half_iters for i in infos)) <= p.n_steps
+    prop.close()
+
+
+def test_zero_iteration_exit_and_zero_state():
+    """||r0|| <= rtol ||b|| at the start of a step: no iteration runs and c is returned unchanged (C4, first test); with
+    c = 0 both norms vanish (nb2 = 0) and the step must still complete with status ok."""
+    p, prop = make("tiny", rtol=0.5)
+    ops, fact = orc.assemble(p), orc.factor_precond(p)
+    c_ref, infos = orc.propagate(p, ops, fact, p.c0, 2)
+    assert [i.half_iters for i in infos] == [0, 0]
+    c = prop.to_device(p.c0)
+    st = prop.propagate(c, p.g_table(2))
+    assert st["steps"] == 2 and st["half_iters"] == 0 and st["status"] == 0
+    assert np.array_equal(c.cpu().numpy(), p.c0) and np.array_equal(c_ref, p.c0)
+    prop.close()
+    p, prop = make("tiny")
+    z = prop.to_device(np.zeros(p.n, dtype=np.complex128))
+    st = prop.propagate(z, p.g_table(3))
+    assert st["steps"] == 3 and st["status"] == 0 and st["half_iters"] == 0
+    assert not np.any(z.cpu().numpy())
+    assert prop.norm(z) == 0.0
+    prop.close()
+
+
+@pytest.mark.parametrize("bw", [7, 27])
+def test_no_coupling_terms(bw):
+    """n_terms = 0 (tdde.h allows it): H = H0, the preconditioner is exact, every step takes the ||s|| exit."""
+    from paper_2512_21697_b200 import Tdde
+    p = tdde_inputs.make_synthetic(name="t0", n_ang=37, n_r=40, bandwidth=bw, n_terms=0, dt=0.01, n_steps=3, rtol=1e-11, seed=8)
+    prop = Tdde(p)
+    ops, fact = orc.assemble(p), orc.factor_precond(p)
+    x = rand_vec(p.n, 3)
+    y = prop.apply(0.5, 1.0 - 1.0j, np.zeros(0), prop.to_device(x)).cpu().numpy()
+    assert rel(y, orc.apply(ops, 0.5, 1.0 - 1.0j, np.zeros(0), x)) <= 1e-12
+    c_ref, infos = orc.propagate(p, ops, fact, p.c0, 3)
+    c = prop.to_device(p.c0)
+    st = prop.propagate(c, np.zeros((3, 0)))
+    assert st["steps"] == 3 and st["half_iters"] == 3 == sum(i.half_iters for i in infos)
+    assert rel(c.cpu().numpy(), c_ref) <= 1e-9
+    prop.close()
+
+
+@pytest.mark.parametrize("bw,T", [(9, 3), (11, 4), (15, 6), (5, 2)])
+def test_untemplated_bandwidths_and_term_counts(bw, T):
+    """Half-bandwidths outside {3, 6, 9, 13} (w = 4, 5, 7, 2) and T = 4, 6: whatever kernels the library picks for them,
+    apply, preconditioner and propagation must match the oracle."""
+    from paper_2512_21697_b200 import Tdde
+    p = tdde_inputs.make_synthetic(name="odd", n_ang=75, n_r=33, bandwidth=bw, n_terms=T, dt=0.005, n_steps=3, rtol=1e-10,
+                                   seed=bw, phase=np.pi / 2, e0=2.0)
+    prop = Tdde(p)
+    ops, fact = orc.assemble(p), orc.factor_precond(p)
+    x = rand_vec(p.n, 6)
+    g = np.linspace(0.4, 1.3, T)
+    y = prop.apply(1.0, 0.5j * p.dt, g, prop.to_device(x)).cpu().numpy()
+    assert rel(y, orc.apply(ops, 1.0, 0.5j * p.dt, g, x)) <= 1e-12
+    z = prop.precond(prop.to_device(x)).cpu().numpy()
+    assert rel(z, orc.apply_precond(fact, x)) <= 1e-12
+    c_ref, infos = orc.propagate(p, ops, fact, p.c0, p.n_steps)
+    c = prop.to_device(p.c0)
+    st = prop.propagate(c, p.g_table(p.n_steps))
+    assert st["steps"] == p.n_steps and rel(c.cpu().numpy(), c_ref) <= 1e-9
+    prop.close()

@@ -157,6 +157,43 @@ def test_p10_sampled_rows_match_csr(tiny_stress, hyd):
     assert np.max(np.abs(ys - ref)) / np.max(np.abs(ref)) < 1e-12
 
 
+def test_p10_apply_panels_vs_dense_kron_and_csr(tiny_stress, hyd):
+    """The panel-streamed full-vector apply (used where the CSR cannot be held) against dense numpy.kron
+    operators (independent of the oracle) on Tiny, and against the CSR apply on the non-banded hydrogen A and on a
+    ragged shape; panel sizes that do not divide N_ang, a panel of one channel and one panel for everything."""
+    p, ops, _ = tiny_stress
+    S, H0, K = dense_operators(p)
+    rng = np.random.default_rng(17)
+    x = rng.standard_normal(p.n) + 1j * rng.standard_normal(p.n)
+    g = np.array([0.3, -0.7, 1.1])
+    alpha, beta = 0.7 - 0.2j, 0.1 + 0.9j
+    ref = alpha * (S @ x) + beta * ((H0 + sum(gl * KL for gl, KL in zip(g, K))) @ x)
+    for panel in (1, 5, 16, 1000):
+        assert rel(orc.apply_panels(p, alpha, beta, g, x, panel=panel), ref) < 1e-13, panel
+    # a zero g_L skips the term; g = 0 leaves the block part
+    g0 = np.array([0.0, 0.5, 0.0])
+    assert rel(orc.apply_panels(p, 1.0, 0.5j, g0, x, panel=7), S @ x + 0.5j * ((H0 + 0.5 * K[1]) @ x)) < 1e-13
+    ph = hyd
+    opsh = orc.assemble(ph)
+    xh = rng.standard_normal(ph.n) + 1j * rng.standard_normal(ph.n)
+    gh = np.linspace(0.2, 0.9, ph.n_terms)
+    assert rel(orc.apply_panels(ph, 1.0, 0.5j, gh, xh, panel=9), orc.apply(opsh, 1.0, 0.5j, gh, xh)) < 1e-13
+    pr = make_synthetic(n_ang=37, n_r=11, bandwidth=13, n_terms=5, dt=0.01, n_steps=1, rtol=1e-10, seed=4)
+    xr = rng.standard_normal(pr.n) + 1j * rng.standard_normal(pr.n)
+    gr = np.linspace(-1.0, 1.0, 5)
+    assert rel(orc.apply_panels(pr, 0.3, 1.0 - 2.0j, gr, xr, panel=16), orc.apply(orc.assemble(pr), 0.3, 1.0 - 2.0j, gr, xr)) < 1e-13
+
+
+def test_cn_step_panels_vs_dense_lu(tiny_stress, tiny_dense):
+    """The matrix-free CN step (cn_step_panels) solves the same dense system as P1."""
+    p, ops, fact = tiny_stress
+    S, H0, K = tiny_dense
+    g = p.g_mid(1)
+    c1, info = orc.cn_step_panels(p, fact, p.c0, g, p.dt, p.rtol, p.max_iter, panel=5)
+    assert info.status == "ok" and info.half_iters >= 2
+    assert rel(c1, dense_step(S, H0, K, g, p.dt, p.c0)) < 1e-10
+
+
 # ----------------------------------------------------------------------------- P8 preconditioner
 def test_p8_precond_vs_dense_solve(tiny):
     p, ops, fact = tiny
