@@ -97,7 +97,7 @@ bool detect_banded(const tdde_config* c, const tdde_term* terms, int* m0, int* m
 extern "C" void tdde_destroy(tdde_handle* h) {
   if (!h) return;
   cudaStreamSynchronize(h->stream);
-  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_pslot, h->d_warp_cls, h->d_Wsp, h->d_Corner, h->d_Schur, h->d_plo, h->d_phi, h->d_rsm, h->d_rsp, h->d_Lcol, h->d_Ucol, h->X, h->r,
+  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_pslot, h->d_warp_cls, h->d_Wsp, h->d_Corner, h->d_Schur, h->d_rsm, h->d_rsp, h->d_Lcol, h->d_Ucol, h->X, h->r,
                   h->rhat, h->p, h->v, h->s, h->t, h->y, h->z, h->c_stage, h->d_st, h->d_st_bench, h->d_partials,
                   h->d_ticket, h->d_g, h->d_g_small, h->d_zero_g};
   for (void* p : ptrs) if (p) cudaFree(p);
@@ -208,6 +208,7 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
       plan = finer;
     }
     h->pc_P = plan.P; h->pc_tile_rows = plan.max_interior();
+    h->pc_base = (n_rad - (plan.P - 1) * w0) / plan.P; h->pc_rem = (n_rad - (plan.P - 1) * w0) % plan.P;
     const size_t ww = (size_t)w0 * w0;
     const int nsep = plan.P - 1;
     std::vector<zc> Wsp(plan.P > 1 ? (size_t)c.n_cls * n_rad * 2 * w0 : 1), Corner(plan.P > 1 ? (size_t)c.n_cls * plan.P * 2 * ww : 1),
@@ -249,8 +250,6 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     if ((rc = dev_upload(&h->d_Wsp, reinterpret_cast<cplx*>(Wsp.data()), Wsp.size(), s))) return rc;
     if ((rc = dev_upload(&h->d_Corner, reinterpret_cast<cplx*>(Corner.data()), Corner.size(), s))) return rc;
     if ((rc = dev_upload(&h->d_Schur, reinterpret_cast<cplx*>(Schur.data()), Schur.size(), s))) return rc;
-    if ((rc = dev_upload(&h->d_plo, plan.lo.data(), plan.lo.size(), s))) return rc;
-    if ((rc = dev_upload(&h->d_phi, plan.hi.data(), plan.hi.size(), s))) return rc;
     if ((rc = dev_upload(&h->d_rsm, (cplx*)nullptr, (size_t)plan.P * w0 * h->ld, s))) return rc;
     if ((rc = dev_upload(&h->d_rsp, (cplx*)nullptr, (size_t)plan.P * w0 * h->ld, s))) return rc;
     CU(cudaStreamSynchronize(s));

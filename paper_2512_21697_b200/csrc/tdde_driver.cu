@@ -68,8 +68,9 @@ int enqueue_precond(tdde_handle* h, const cplx* x, cplx* y, const SolverState* s
   p.x = x; p.y = y; p.n_ang = h->cfg.n_ang; p.n_rad = h->cfg.n_rad; p.ld = h->ld; p.w = h->cfg.w0;
   p.cls = h->d_cls; p.Lcol = h->d_Lcol; p.Ucol = h->d_Ucol; p.st = st;
   p.slot = h->d_pslot; p.warp_cls = h->d_warp_cls;
-  p.P = h->pc_P; p.tile_rows = h->pc_tile_rows; p.plo = h->d_plo; p.phi = h->d_phi;
+  p.P = h->pc_P; p.tile_rows = h->pc_tile_rows; p.int_base = h->pc_base; p.int_rem = h->pc_rem;
   p.Wsp = h->d_Wsp; p.Corner = h->d_Corner; p.Schur = h->d_Schur; p.rsm = h->d_rsm; p.rsp = h->d_rsp;
+  p.aslot = h->d_slot; p.cta_cls = h->d_cta_cls;
   int rc = launch_precond(p, h->stream);
   if (rc == -2) return tdde_cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(precond)");
   if (rc < 0) return TDDE_EINVAL;

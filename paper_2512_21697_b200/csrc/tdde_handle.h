@@ -40,7 +40,7 @@ struct tdde_handle {
   cplx *d_Lcol = nullptr, *d_Ucol = nullptr; // preconditioner factors
   int *d_pslot = nullptr, *d_warp_cls = nullptr;
   int pc_P = 1, pc_tile_rows = 0;            // partitioned solve (tdde_partition.h)
-  int *d_plo = nullptr, *d_phi = nullptr;
+  int pc_base = 0, pc_rem = 0;               // interior q: pc_base + (q < pc_rem) rows
   cplx *d_Wsp = nullptr, *d_Corner = nullptr, *d_Schur = nullptr, *d_rsm = nullptr, *d_rsp = nullptr;
   double lu_growth = 1.0;                    // largest element growth of the unpivoted interior LUs over all classes
 

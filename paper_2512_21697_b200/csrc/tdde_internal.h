@@ -32,7 +32,7 @@
 #ifndef TDDE_AP_MAXC
 #define TDDE_AP_MAXC 16    // banded apply: distinct kappa-classes per CTA staged in shared memory
 #endif
-#define TDDE_PC_MAXC 4      // preconditioner: distinct kappa-classes per warp staged in shared memory
+#define TDDE_PC_MAXC 2      // preconditioner: distinct kappa-classes per warp staged in shared memory
 // half-bandwidths the preconditioner kernels are instantiated for (others <= 32 take the runtime-w two-sweep kernel)
 #define TDDE_PC_WIDTHS(X) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13)
 #define TDDE_PC_MAXW 13
@@ -138,15 +138,22 @@ struct PrecArgs {
   // partitioned solve (tdde_partition.h); P == 1: plain LU over all rows
   int P;                   // interiors
   int tile_rows;           // longest interior = rows of the shared-memory tile
-  const int* plo;          // device [P]: interior q = rows [plo[q], phi[q]); separator q = rows [phi[q], phi[q] + w)
-  const int* phi;
+  int int_base, int_rem;   // interior q has int_base + (q < int_rem) rows and starts at row q (int_base + w) + min(q, int_rem);
+                           // separator q = the w rows after interior q (make_partition_plan)
   const cplx* Wsp;         // [n_cls][n_rad][2w] left spikes
   const cplx* Corner;      // [n_cls][P][2][w][w] corner blocks of A_IS
   const cplx* Schur;       // [n_cls][P-1][3][w][w] block Thomas factors of the Schur complement
-  cplx* rsm;               // scratch [P][w][ld]: spike products towards the separator before each interior
-  cplx* rsp;               // scratch [P][w][ld]: ... after each interior; reused for the forward-eliminated Schur rhs
+  cplx* rsm;               // scratch [P][w][ld]: P1 -> P2: spike products towards the separator before each interior;
+                           //   P2 -> P3: A_IS x_S for the first w rows of each interior
+  cplx* rsp;               // scratch [P][w][ld]: P1 -> P2: spike products towards the separator after each interior; inside P2 the
+                           //   forward-eliminated Schur rhs; P2 -> P3: A_IS x_S for the last w rows of each interior
+  const int* aslot;        // [ld] the apply's per-CTA class slot (128-channel groups), used by k_precond_spikes
+  const int* cta_cls;      // [n_cta][TDDE_AP_MAXC]
   const SolverState* st;   // nullable guard
 };
+
+__host__ __device__ inline int pc_lo(const PrecArgs& p, int q) { return q * (p.int_base + p.w) + (q < p.int_rem ? q : p.int_rem); }
+__host__ __device__ inline int pc_len(const PrecArgs& p, int q) { return p.int_base + (q < p.int_rem ? 1 : 0); }
 
 // launchers (each returns the number of kernels launched, or -1 if no instantiation fits)
 int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, int ng, cudaStream_t s);

@@ -182,7 +182,12 @@ bool build_partitioned_factors(const std::vector<zc>& Mrow, const PartitionPlan&
     zc* out = Schur + (size_t)j * 3 * ww;
     std::copy(Lb.begin(), Lb.end(), out);
     std::copy(Dinv_prev.begin(), Dinv_prev.end(), out + ww);
-    std::copy(C.begin(), C.end(), out + 2 * ww);
+    for (int a = 0; a < w; ++a)                                   // G_j = D'^-1_j C_j: x_j = D'^-1_j r'_j - G_j x_{j+1}
+      for (int b2 = 0; b2 < w; ++b2) {
+        zc acc(0, 0);
+        for (int k = 0; k < w; ++k) acc += Dinv_prev[a * w + k] * C[k * w + b2];
+        out[2 * ww + a * w + b2] = acc;
+      }
     Cprev = C;
   }
   return true;
@@ -213,41 +218,53 @@ extern "C" int tdde_selftest_partition(int32_t n, int32_t w, int32_t P, uint32_t
   if (!build_partitioned_factors(Mrow, pl, Lc.data(), Uc.data(), Wsp.data(), Corner.data(), Sch.data(), &growth)) return TDDE_ESINGULAR;
   std::vector<zc> b(n), y(n, zc(0, 0));
   for (int i = 0; i < n; ++i) b[i] = zc(rnd(), rnd());
+  std::vector<zc> rsm((size_t)Pp * w, zc(0, 0)), rsp((size_t)Pp * w, zc(0, 0));
   if (Pp > 1) {
     // kernel P1: per interior, the spike dot products for the separator before (minus) and after (plus)
-    std::vector<zc> rsm((size_t)Pp * w, zc(0, 0)), rsp((size_t)Pp * w, zc(0, 0));
     for (int q = 0; q < Pp; ++q)
       for (int i = pl.lo[q]; i < pl.hi[q]; ++i)
         for (int c = 0; c < w; ++c) {
           rsm[(size_t)q * w + c] += Wsp[(size_t)i * 2 * w + c] * b[i];
           rsp[(size_t)q * w + c] += Wsp[(size_t)i * 2 * w + w + c] * b[i];
         }
-    // kernel P2: block Thomas over the separators
-    std::vector<zc> rp((size_t)(Pp - 1) * w), prev(w, zc(0, 0)), cur(w), xn(w, zc(0, 0));
+    // kernel P2: block Thomas over the separators.  Forward: r'_j = r_j - Lb_j r'_{j-1}, z_j = D'^-1_j r'_j (kept in rsp);
+    // backward: x_j = z_j - G_j x_{j+1}
+    std::vector<zc> prev(w, zc(0, 0)), cur(w), xn(w, zc(0, 0));
     for (int j = 0; j + 1 < Pp; ++j) {
       const zc* Lb = Sch.data() + (size_t)j * 3 * ww;
+      const zc* Di = Lb + ww;
       for (int c = 0; c < w; ++c) {
         zc r = b[pl.hi[j] + c] - rsp[(size_t)j * w + c] - rsm[(size_t)(j + 1) * w + c];
         for (int k = 0; k < w; ++k) r -= Lb[c * w + k] * prev[k];
         cur[c] = r;
       }
-      for (int c = 0; c < w; ++c) rp[(size_t)j * w + c] = prev[c] = cur[c];
+      for (int c = 0; c < w; ++c) prev[c] = cur[c];
+      for (int c = 0; c < w; ++c) {
+        zc z(0, 0);
+        for (int k = 0; k < w; ++k) z += Di[c * w + k] * prev[k];
+        rsp[(size_t)j * w + c] = z;
+      }
     }
     for (int j = Pp - 2; j >= 0; --j) {
-      const zc* Di = Sch.data() + (size_t)j * 3 * ww + ww;
-      const zc* Cj = Di + ww;
+      const zc* G = Sch.data() + (size_t)j * 3 * ww + 2 * ww;
       for (int c = 0; c < w; ++c) {
-        zc r = rp[(size_t)j * w + c];
-        for (int k = 0; k < w; ++k) r -= Cj[c * w + k] * xn[k];
-        cur[c] = r;
+        zc x = rsp[(size_t)j * w + c];
+        for (int k = 0; k < w; ++k) x -= G[c * w + k] * xn[k];
+        cur[c] = x;
       }
-      for (int c = 0; c < w; ++c) {
-        zc x(0, 0);
-        for (int k = 0; k < w; ++k) x += Di[c * w + k] * cur[k];
-        y[pl.hi[j] + c] = x;
-      }
-      for (int c = 0; c < w; ++c) xn[c] = y[pl.hi[j] + c];
+      for (int c = 0; c < w; ++c) xn[c] = y[pl.hi[j] + c] = cur[c];
     }
+    // kernel P2b: A_IS x_S for the interiors next to each separator
+    for (int j = 0; j + 1 < Pp; ++j)
+      for (int c = 0; c < w; ++c) {
+        zc ct(0, 0), cb(0, 0);
+        for (int k = 0; k < w; ++k) {
+          ct += Corner[((size_t)(j + 1) * 2 + 0) * ww + c * w + k] * y[pl.hi[j] + k];
+          cb += Corner[((size_t)j * 2 + 1) * ww + c * w + k] * y[pl.hi[j] + k];
+        }
+        rsm[(size_t)(j + 1) * w + c] = ct;
+        rsp[(size_t)j * w + c] = cb;
+      }
   }
   // kernel P3: per interior, corner-corrected right-hand side, then forward and backward sweep in column form
   for (int q = 0; q < Pp; ++q) {
@@ -255,11 +272,9 @@ extern "C" int tdde_selftest_partition(int32_t n, int32_t w, int32_t P, uint32_t
     std::vector<zc> tile(len);
     for (int r = 0; r < len; ++r) tile[r] = b[lo + r];
     if (q > 0)
-      for (int r = 0; r < w; ++r)
-        for (int c = 0; c < w; ++c) tile[r] -= Corner[((size_t)q * 2 + 0) * ww + r * w + c] * y[pl.hi[q - 1] + c];
+      for (int r = 0; r < w; ++r) tile[r] -= rsm[(size_t)q * w + r];
     if (q + 1 < Pp)
-      for (int r = 0; r < w; ++r)
-        for (int c = 0; c < w; ++c) tile[len - w + r] -= Corner[((size_t)q * 2 + 1) * ww + r * w + c] * y[hi + c];
+      for (int r = 0; r < w; ++r) tile[len - w + r] -= rsp[(size_t)q * w + r];
     std::vector<zc> pw(w + 1, zc(0, 0));
     for (int r = 0; r < len; ++r) {
       const int i = lo + r;

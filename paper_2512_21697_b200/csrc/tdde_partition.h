@@ -41,7 +41,7 @@ int partitions_for_rows(int n, int w, int rows);
 //   Lcol  [n][w], Ucol [n][w+1]   LU of the interiors in the layout of tdde_precond.cu (separator rows = identity)
 //   Wsp   [n][2w]                 interior row i of interior q: [c] = W[separator q-1, row c][i], [w+c] = W[separator q, row c][i]
 //   Corner[P][2][w][w]            A_IS corners: [q][0][r][c] = M[lo_q + r][hi_{q-1} + c], [q][1][r][c] = M[hi_q - w + r][hi_q + c]
-//   Schur [P-1][3][w][w]          block Thomas of Sc: [j][0] = B_j D'_{j-1}^{-1}, [j][1] = D'_j^{-1}, [j][2] = C_j (row-major)
+//   Schur [P-1][3][w][w]          block Thomas of Sc: [j][0] = B_j D'_{j-1}^{-1}, [j][1] = D'_j^{-1}, [j][2] = D'_j^{-1} C_j (row-major)
 // growth (nullable): max |L_ij|, |U_ij| over the interiors divided by max |M_ij| (element growth of the unpivoted LU).
 // Returns false on a zero / non-finite pivot.
 bool build_partitioned_factors(const std::vector<zc>& Mrow, const PartitionPlan& plan, zc* Lcol, zc* Ucol, zc* Wsp,

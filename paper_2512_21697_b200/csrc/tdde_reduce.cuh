@@ -16,6 +16,11 @@ __device__ __forceinline__ void cfma(cplx& acc, cplx a, cplx b) {
   acc.x = fma(a.x, b.x, acc.x); acc.x = fma(-a.y, b.y, acc.x);
   acc.y = fma(a.x, b.y, acc.y); acc.y = fma(a.y, b.x, acc.y);
 }
+// acc -= a * b  (4 DFMA; the negations are operand modifiers)
+__device__ __forceinline__ void cfms(cplx& acc, cplx a, cplx b) {
+  acc.x = fma(-a.x, b.x, acc.x); acc.x = fma(a.y, b.y, acc.x);
+  acc.y = fma(-a.x, b.y, acc.y); acc.y = fma(-a.y, b.x, acc.y);
+}
 // acc += conj(a) * b
 __device__ __forceinline__ void cfma_conj(cplx& acc, cplx a, cplx b) {
   acc.x = fma(a.x, b.x, acc.x); acc.x = fma(a.y, b.y, acc.x);
