@@ -47,6 +47,9 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                "l"(src), "r"(bytes), "r"(smem_u32(bar))
                : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   uint32_t ok;
   do {
@@ -70,8 +73,12 @@ struct ApplyPlan {
   static constexpr int XW = AP_NC + 2 * MAXM;
   // rows per stage: the two-group variant (one CTA per SM) takes twice as many when the shared memory allows,
   // which halves the number of CTA barriers (measured: HBM-scale 2.41 -> 2.25 ms)
+  // BLK == false (in-iteration applies): the fused-dot operand and the vector replacing the block part reach the row loop
+  // through a per-thread cp.async double buffer instead of plain global loads inside it
+  static constexpr bool VST = !BLK && T > 0;
   __host__ __device__ static constexpr size_t smem_for(int jc) {
-    return (size_t)(3 * (jc * T * ND + (BLK ? AP_MAXC * jc * ND : 0) + jc * XW) + ((T > 0 && NG == 2) ? 2 * jc * AP_NC : 0)) * sizeof(cplx) + 64;
+    return (size_t)(3 * (jc * T * ND + (BLK ? AP_MAXC * jc * ND : 0) + jc * XW) + ((T > 0 && NG == 2) ? 2 * jc * AP_NC : 0) +
+                    (VST ? 4 * jc * AP_NC : 0)) * sizeof(cplx) + 64;
   }
   static constexpr int JC = (NG == 2 && smem_for(2 * AP_JC) <= 220 * 1024) ? 2 * AP_JC : AP_JC;
   static constexpr int RS = JC * T * ND;                    // complex elements
@@ -79,8 +86,9 @@ struct ApplyPlan {
   static constexpr int XS = JC * XW;
   static constexpr int STAGE = RS + BS + XS;
   static constexpr int PS = (T > 0 && NG == 2) ? 2 * JC * AP_NC : 0;
+  static constexpr int VS = VST ? 4 * JC * AP_NC : 0;       // [2 buffers][aux, addv][JC][AP_NC]
   static constexpr int NSTAGE = 3;
-  static constexpr size_t SMEM = (size_t)(NSTAGE * STAGE + PS) * sizeof(cplx) + 64;
+  static constexpr size_t SMEM = (size_t)(NSTAGE * STAGE + PS + VS) * sizeof(cplx) + 64;
   // Term split: the terms of one channel are shared between two warp groups so that each thread keeps only about
   // half of the A_L registers (4 warps per SM sub-partition instead of 2).  Group 0 also owns the block part, the
   // write-out and the fused inner products.  Greedy balance of complex FMAs per row, largest term first.
@@ -105,7 +113,10 @@ struct ApplyCommon {
   bool lane_ok;
   cplx* stage_base;
   cplx* Ps;
-  uint64_t* full;
+  cplx* Vs;
+  uint64_t* full;       // [NSTAGE] TMA landed
+  uint64_t* pfull;      // [2] group 1 has published its partial rows of a chunk
+  uint64_t* pempty;     // [2] group 0 has consumed them
   const cplx* blk_g;
 };
 
@@ -139,90 +150,118 @@ __device__ __forceinline__ void apply_group(const ApplyArgs& p, const ApplyCommo
 #pragma unroll
   for (int e = 0; e < ND; ++e) yw[e] = make_double2(0, 0);
 
-  // Time is cut into slots separated by one CTA barrier.  In slot s group 1 works on chunk s and group 0 on chunk
-  // s - 1, so group 0 finds group 1's partial rows of its chunk already published and can finish every output row
-  // (sum, store, fused inner products) the moment its own part is complete.
-  for (int s = 0; s < k.nchunks + (NG - 1); ++s) {
-    const int c = (G == 1 || NG == 1) ? s : s - 1;
-    if (c >= 0 && c < k.nchunks) {
-      const cplx* st = k.stage_base + (size_t)(c % PL::NSTAGE) * PL::STAGE;
-      cplx* ps = k.Ps + (size_t)(c & 1) * JC * AP_NC;
+  // Group 1 runs ahead: it publishes its partial rows of chunk c in Ps[c & 1] and signals pfull[c & 1]; group 0 waits for that,
+  // finishes every output row of the chunk (sum, store, fused inner products) and signals pempty[c & 1].  Nobody waits at a
+  // CTA-wide barrier: group 1 only blocks when it is two chunks ahead, group 0 only on group 1's chunk.  A stage buffer is
+  // refilled (chunk c + 3) by group 0's first thread once all of group 0 is done with chunk c -- group 1 then is, too.
+  constexpr bool VST = PL::VST;
+  auto vfetch = [&](int c) {                                   // G == 0: aux / addv rows completed by chunk c -> Vs[c & 1]
+    if (c < k.nchunks) {
       const int jc0 = k.jlo + c * JC;
-      const int nr_real = min(JC, k.jhi - jc0);               // rows with data; later rows of the chunk are virtual
-      const int nr_all = min(JC, k.jend - jc0);
-      if (nr_real > 0) mbar_wait(&k.full[c % PL::NSTAGE], (c / PL::NSTAGE) & 1);
-#pragma unroll RU
-      for (int r = 0; r < nr_all; ++r) {
-        const int i = jc0 + r - W;                            // the output row completed by input row jc0 + r
-        const bool emit = (G == 0) && (i >= k.i0) && k.lane_ok;
-        cplx ax = make_double2(0, 0), pg = make_double2(0, 0);
-        if (G == 0) {
-          if (emit && p.aux) ax = p.aux[(size_t)i * ld + k.a];
-          if (SPLIT) pg = ps[r * AP_NC + k.tid];
-          if (!BLK && emit) pg = cadd(pg, p.addv[(size_t)i * ld + k.a]);   // block part replaced by a known vector
+      cplx* vb = k.Vs + (size_t)(c & 1) * 2 * JC * AP_NC + k.tid;
+#pragma unroll
+      for (int r = 0; r < JC; ++r) {
+        const int i = jc0 + r - W;
+        if (i >= k.i0 && i < k.i1 && k.lane_ok) {
+          if (p.aux) cp_async16(vb + r * AP_NC, p.aux + (size_t)i * ld + k.a);
+          cp_async16(vb + (JC + r) * AP_NC, p.addv + (size_t)i * ld + k.a);
         }
-        if (r < nr_real) {
-          const cplx* xs = st + PL::RS + PL::BS + (size_t)r * XW + k.tid + MAXM;
-          if (G == 0 && BLK) {
-            const cplx x0 = xs[0];
-            if (k.slot >= 0) {
-              const cplx* bc = st + PL::RS + ((size_t)k.slot * JC + r) * ND;
-#pragma unroll
-              for (int e = 0; e < ND; ++e) cfma(yw[e], bc[e], x0);
-            } else {
-              const cplx* bc = k.blk_g + (size_t)(jc0 + r) * ND;
-#pragma unroll
-              for (int e = 0; e < ND; ++e) cfma(yw[e], __ldg(bc + e), x0);
-            }
-          }
-          if (T > 0 && GM > 0) {
-            cplx z[T > 0 ? T : 1];
-#pragma unroll
-            for (int L = 0; L < T; ++L) z[L] = make_double2(0, 0);
-#pragma unroll
-            for (int o = -GM; o <= GM; ++o) {
-              if (o == 0) continue;
-              const cplx xo = xs[o];
-#pragma unroll
-              for (int L = 0; L < T; ++L) {
-                if (PL::mine(G, L) && SH::m(L) >= (o < 0 ? -o : o)) {
-                  // slot order within a term: o = -m..-1 -> q = o + m ; o = 1..m -> q = m + o - 1
-                  const int q = o < 0 ? o + SH::m(L) : SH::m(L) + o - 1;
-                  cfma(z[L], Areg[SH::slot0(L) + q], xo);
-                }
-              }
-            }
-#pragma unroll
-            for (int L = 0; L < T; ++L) {
-              if (!PL::mine(G, L)) continue;
-              const cplx* rc = st + ((size_t)r * T + L) * ND;  // warp-uniform: broadcast LDS.128
-#pragma unroll
-              for (int e = 0; e < ND; ++e) cfma(yw[e], rc[e], z[L]);
-            }
-          }
-        }
-        if (G == 1) {
-          if (SPLIT) ps[r * AP_NC + k.tid] = yw[0];
-        } else if (emit) {
-          cplx yv = cadd(yw[0], pg);
-          if (p.emode == 2) {                                 // ||b||^2 = ||S c + r0 / 2||^2, nothing stored
-            yv.x = fma(0.5, ax.x, yv.x); yv.y = fma(0.5, ax.y, yv.y);
-          } else {
-            if (p.emode == 1) { yv = cmul(p.oscale, yv); p.y2[(size_t)i * ld + k.a] = yv; }
-            p.y[(size_t)i * ld + k.a] = yv;
-            cfma_conj(d0, ax, yv);
-          }
-          d1 = fma(yv.x, yv.x, d1); d1 = fma(yv.y, yv.y, d1);
-        }
-#pragma unroll
-        for (int e = 0; e < ND - 1; ++e) yw[e] = yw[e + 1];
-        yw[ND - 1] = make_double2(0, 0);
       }
     }
-    // both groups are done with their chunks of this slot; group 1's partial rows are published
-    asm volatile("bar.sync 1, %0;" ::"n"(NG * AP_NC) : "memory");
-    if (G == 0 && k.tid == 0 && s + 2 < k.nchunks) issue(s + 2);
+    cp_async_commit();
+  };
+  if (G == 0 && VST) vfetch(0);
+  for (int c = 0; c < k.nchunks; ++c) {
+    const cplx* st = k.stage_base + (size_t)(c % PL::NSTAGE) * PL::STAGE;
+    cplx* ps = k.Ps + (size_t)(c & 1) * JC * AP_NC;
+    const cplx* vs = k.Vs + (size_t)(c & 1) * 2 * JC * AP_NC + k.tid;
+    const int jc0 = k.jlo + c * JC;
+    const int nr_real = min(JC, k.jhi - jc0);               // rows with data; later rows of the chunk are virtual
+    const int nr_all = min(JC, k.jend - jc0);
+    if (G == 0 && VST) { vfetch(c + 1); cp_async_wait<1>(); }
+    if (nr_real > 0) mbar_wait(&k.full[c % PL::NSTAGE], (c / PL::NSTAGE) & 1);
+    if (SPLIT && G == 1 && c >= 2) mbar_wait(&k.pempty[c & 1], ((c >> 1) - 1) & 1);
+    if (SPLIT && G == 0) mbar_wait(&k.pfull[c & 1], (c >> 1) & 1);
+#pragma unroll RU
+    for (int r = 0; r < nr_all; ++r) {
+      const int i = jc0 + r - W;                            // the output row completed by input row jc0 + r
+      const bool emit = (G == 0) && (i >= k.i0) && k.lane_ok;
+      cplx ax = make_double2(0, 0), pg = make_double2(0, 0);
+      if (G == 0) {
+        if (VST) {
+          if (emit && p.aux) ax = vs[r * AP_NC];
+        } else {
+          if (emit && p.aux) ax = p.aux[(size_t)i * ld + k.a];
+        }
+        if (SPLIT) pg = ps[r * AP_NC + k.tid];
+        if (VST && emit) pg = cadd(pg, vs[(JC + r) * AP_NC]);   // block part replaced by a known vector
+      }
+      if (r < nr_real) {
+        const cplx* xs = st + PL::RS + PL::BS + (size_t)r * XW + k.tid + MAXM;
+        if (G == 0 && BLK) {
+          const cplx x0 = xs[0];
+          if (k.slot >= 0) {
+            const cplx* bc = st + PL::RS + ((size_t)k.slot * JC + r) * ND;
+#pragma unroll
+            for (int e = 0; e < ND; ++e) cfma(yw[e], bc[e], x0);
+          } else {
+            const cplx* bc = k.blk_g + (size_t)(jc0 + r) * ND;
+#pragma unroll
+            for (int e = 0; e < ND; ++e) cfma(yw[e], __ldg(bc + e), x0);
+          }
+        }
+        if (T > 0 && GM > 0) {
+          cplx z[T > 0 ? T : 1];
+#pragma unroll
+          for (int L = 0; L < T; ++L) z[L] = make_double2(0, 0);
+#pragma unroll
+          for (int o = -GM; o <= GM; ++o) {
+            if (o == 0) continue;
+            const cplx xo = xs[o];
+#pragma unroll
+            for (int L = 0; L < T; ++L) {
+              if (PL::mine(G, L) && SH::m(L) >= (o < 0 ? -o : o)) {
+                // slot order within a term: o = -m..-1 -> q = o + m ; o = 1..m -> q = m + o - 1
+                const int q = o < 0 ? o + SH::m(L) : SH::m(L) + o - 1;
+                cfma(z[L], Areg[SH::slot0(L) + q], xo);
+              }
+            }
+          }
+#pragma unroll
+          for (int L = 0; L < T; ++L) {
+            if (!PL::mine(G, L)) continue;
+            const cplx* rc = st + ((size_t)r * T + L) * ND;  // warp-uniform: broadcast LDS.128
+#pragma unroll
+            for (int e = 0; e < ND; ++e) cfma(yw[e], rc[e], z[L]);
+          }
+        }
+      }
+      if (G == 1) {
+        if (SPLIT) ps[r * AP_NC + k.tid] = yw[0];
+      } else if (emit) {
+        cplx yv = cadd(yw[0], pg);
+        if (p.emode == 2) {                                 // ||b||^2 = ||S c + r0 / 2||^2, nothing stored
+          yv.x = fma(0.5, ax.x, yv.x); yv.y = fma(0.5, ax.y, yv.y);
+        } else {
+          if (p.emode == 1) { yv = cmul(p.oscale, yv); p.y2[(size_t)i * ld + k.a] = yv; }
+          p.y[(size_t)i * ld + k.a] = yv;
+          cfma_conj(d0, ax, yv);
+        }
+        d1 = fma(yv.x, yv.x, d1); d1 = fma(yv.y, yv.y, d1);
+      }
+#pragma unroll
+      for (int e = 0; e < ND - 1; ++e) yw[e] = yw[e + 1];
+      yw[ND - 1] = make_double2(0, 0);
+    }
+    if (G == 1) {
+      if (SPLIT) mbar_arrive(&k.pfull[c & 1]);
+    } else {
+      if (SPLIT) mbar_arrive(&k.pempty[c & 1]);
+      asm volatile("bar.sync 1, %0;" ::"n"(AP_NC) : "memory");   // group 0 only: everybody is done with stage c % NSTAGE
+      if (k.tid == 0 && c + PL::NSTAGE < k.nchunks) issue(c + PL::NSTAGE);
+    }
   }
+  if (G == 0 && VST) cp_async_wait<0>();
 }
 
 template <int T, int M0, int MS, int W, int NG, bool BLK>
@@ -237,7 +276,10 @@ __global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB
   ApplyCommon k;
   k.stage_base = reinterpret_cast<cplx*>(smem_raw);
   k.Ps = k.stage_base + (size_t)PL::NSTAGE * PL::STAGE;
-  k.full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)(PL::NSTAGE * PL::STAGE + PL::PS) * sizeof(cplx));
+  k.Vs = k.Ps + PL::PS;
+  k.full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)(PL::NSTAGE * PL::STAGE + PL::PS + PL::VS) * sizeof(cplx));
+  k.pfull = k.full + PL::NSTAGE;
+  k.pempty = k.pfull + 2;
 
   const int grp = threadIdx.x / AP_NC;                       // warp-uniform
   k.tid = threadIdx.x % AP_NC;
@@ -269,6 +311,7 @@ __global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB
   }
   if (threadIdx.x == 0) {
     for (int q = 0; q < PL::NSTAGE; ++q) mbar_init(&full[q], 1);
+    for (int q = 0; q < 2; ++q) { mbar_init(&k.pfull[q], AP_NC); mbar_init(&k.pempty[q], AP_NC); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -308,8 +351,7 @@ __global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB
     }
   };
   if (threadIdx.x == 0) {
-    issue(0);
-    if (k.nchunks > 1) issue(1);
+    for (int c = 0; c < PL::NSTAGE && c < k.nchunks; ++c) issue(c);
   }
 
   cplx d0 = make_double2(0, 0);

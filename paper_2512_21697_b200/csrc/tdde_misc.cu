@@ -38,7 +38,7 @@ extern "C" int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, con
   int rc = 0;
   auto once = [&]() -> int {
     switch (which) {
-      case 0: return enqueue_apply(h, h->y, h->v, h->rhat, BLK_MP, itau, true, h->d_g_small, nullptr, 0, FIN_NONE, sb, h->p);
+      case 0: return enqueue_apply(h, h->y, h->v, h->rhat, BLK_MP, itau, true, h->d_g_small, nullptr, 0, FIN_ALPHA, sb, h->p);   // as the iteration runs it
       case 1: return enqueue_precond(h, h->p, h->y, nullptr);
       case 2: h->launches += launch_vec_p(make_vec_args(h, sb, FIN_NONE), s); return 0;
       case 3: h->launches += launch_vec_s(make_vec_args(h, sb, FIN_NONE), s); return 0;

@@ -41,6 +41,14 @@ __device__ __forceinline__ bool cbad(cplx a) {
   return !(isfinite(a.x) && isfinite(a.y)) || m < TDDE_TINY;
 }
 
+// per-thread asynchronous 16-byte copies global -> shared (LDGSTS)
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 __device__ __forceinline__ bool solver_idle(const SolverState* st) {
   // uniform over the grid: all three are only written by finalisers of earlier kernels
   return st->done | st->stalled | (st->status != 0);
