@@ -146,7 +146,8 @@ int tdde_selftest_partition(int32_t n, int32_t w, int32_t P, uint32_t seed, doub
 /* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
 int64_t tdde_launch_count(const tdde_handle* h);
 
-/* Which operator-apply kernel the handle uses: 1 = banded-A register-resident fast path, 0 = generic CSR path. */
+/* Which operator-apply kernel the handle uses: 1 = banded A_L held in registers, 2 = general sparse A_L staged in shared memory
+ * (x tile by TMA), 0 = unstaged generic CSR fall-back. */
 int tdde_apply_path(const tdde_handle* h);
 
 void        tdde_destroy(tdde_handle* h);          /* NULL is allowed */

@@ -246,7 +246,7 @@ class Tdde:
 
     @property
     def apply_path(self) -> str:
-        return "banded" if self.lib.tdde_apply_path(self.h) == 1 else "generic"
+        return {1: "banded", 2: "staged", 0: "generic"}.get(self.lib.tdde_apply_path(self.h), "unknown")
 
     def close(self):
         if getattr(self, "h", None):

@@ -19,9 +19,9 @@ ROOT = os.path.dirname(HERE)
 INCLUDE = os.path.join(ROOT, "include")
 OUT = os.environ.get("TDDE_LIB_OUT", os.path.join(HERE, "libtdde.so"))      # overrides: build-variant experiments
 EXTRA = os.environ.get("TDDE_NVCC_FLAGS", "").split()
-SOURCES = ["tdde_apply.cu", "tdde_vec.cu", "tdde_precond.cu", "tdde_partition.cu", "tdde_create.cu", "tdde_driver.cu", "tdde_misc.cu", "tdde_paper_variant.cu"]
+SOURCES = ["tdde_apply.cu", "tdde_apply_sparse.cu", "tdde_vec.cu", "tdde_precond.cu", "tdde_partition.cu", "tdde_create.cu", "tdde_driver.cu", "tdde_misc.cu", "tdde_paper_variant.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
-FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--use_fast_math=false"]
+FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
 
 def _nvcc() -> str:
@@ -45,7 +45,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     bdir = os.path.join(CSRC, "build" + ("_" + "".join(c for c in "".join(EXTRA) if c.isalnum()) if EXTRA else ""))
     os.makedirs(bdir, exist_ok=True)
     hdr_t = _newest_header()
-    flags = [f for f in FLAGS if f != "--use_fast_math=false"]
+    flags = list(FLAGS)
     jobs = []
     objs = []
     for src in SOURCES:

@@ -14,6 +14,7 @@
 //   * the 2W+1 pending outputs y[j-W .. j+W] are a register window; when row j has been consumed output
 //     j-W is complete, is written once (coalesced) and enters the fused inner products.
 // This kernel is FP64-FMA bound (27-52 flop per HBM byte), not HBM bound.
+#include <algorithm>
 #include "tdde_reduce.cuh"
 
 #define AP_NT 128            // generic kernel: threads per block
@@ -361,17 +362,21 @@ __global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB
   if (p.red.fin != FIN_NONE) grid_reduce_finalize<AP_BT>(d0.x, d0.y, d1, p.red);
 }
 
-// ---- generic path: arbitrary CSR A_L, arbitrary per-term bandwidths; one thread per output element. ----
-// Correct for any input the ABI accepts (e.g. the selection-rule-sparse hydrogen coupling); not tuned.
+// ---- generic path: arbitrary CSR A_L, arbitrary per-term bandwidths; one thread per output element, no staging. ----
+// Correct for any input the ABI accepts; the fall-back when neither structured kernel applies.  The grid is bounded
+// (blocks stride over (row, channel-block) pairs), so the per-block reduction scratch can never overflow.
 __global__ void __launch_bounds__(AP_NT) k_apply_generic(const ApplyArgs p) {
   if (p.guard == 1 && solver_idle(p.red.st)) return;
   if (p.guard == 2 && (p.red.st->stalled | (p.red.st->status != 0))) return;
-  const int a = blockIdx.x * AP_NT + threadIdx.x;
-  const int i = blockIdx.y;
   const int ld = p.ld, n_rad = p.n_rad;
+  const int cb = (ld + AP_NT - 1) / AP_NT;
+  const long long nwork = (long long)cb * n_rad;
   cplx d0 = make_double2(0, 0);
   double d1 = 0;
-  if (a < ld) {
+  for (long long wk = blockIdx.x; wk < nwork; wk += gridDim.x) {
+    const int a = (int)(wk % cb) * AP_NT + threadIdx.x;
+    const int i = (int)(wk / cb);
+    if (a >= ld) continue;
     cplx acc = make_double2(0, 0);
     if (a < p.n_ang) {
       const int w0 = p.w0, nd0 = 2 * w0 + 1;
@@ -428,13 +433,15 @@ bool apply_banded_available(int T, int m0, int mstep, int W) {
 
 template <int T, int M0, int MS, int W, int NG, bool BLK>
 static int launch_banded_one(const ApplyArgs& a, dim3 grid, cudaStream_t s) {
-  static bool attr_set = false;
+  static bool attr_set[64] = {};                            // per device: the attribute belongs to the function on one device
   const size_t smem = ApplyPlan<T, M0, MS, W, NG, BLK>::SMEM;
-  if (!attr_set) {
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev < 0 || dev >= 64 || !attr_set[dev]) {
     if (cudaFuncSetAttribute(k_apply_banded<T, M0, MS, W, NG, BLK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) !=
         cudaSuccess)
       return -2;
-    attr_set = true;
+    if (dev >= 0 && dev < 64) attr_set[dev] = true;
   }
   k_apply_banded<T, M0, MS, W, NG, BLK><<<grid, NG * AP_NC, smem, s>>>(a);
   return 1;
@@ -456,8 +463,10 @@ int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, int
   return -1;
 }
 
-int launch_apply_generic(const ApplyArgs& a, cudaStream_t s) {
-  dim3 grid((a.ld + AP_NT - 1) / AP_NT, a.n_rad);
+int launch_apply_generic(const ApplyArgs& a, int num_sms, cudaStream_t s) {
+  const long long nwork = (long long)((a.ld + AP_NT - 1) / AP_NT) * a.n_rad;
+  const long long cap = std::min<long long>((long long)num_sms * 16, TDDE_MAX_PARTIAL_BLOCKS);
+  const int grid = (int)std::max<long long>(1, std::min(nwork, cap));
   k_apply_generic<<<grid, AP_NT, 0, s>>>(a);
   return 1;
 }

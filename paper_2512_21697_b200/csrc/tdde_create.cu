@@ -37,6 +37,16 @@ void row_to_col_band(const zc* row, zc* col, int n, int w) {
     }
 }
 
+// same, into a wider column band of half-width W >= w (entries beyond w are zero)
+void row_to_col_band_padded(const zc* row, zc* col, int n, int w, int W) {
+  const int nd = 2 * w + 1, ND = 2 * W + 1;
+  for (int j = 0; j < n; ++j)
+    for (int e = 0; e < ND; ++e) {
+      const int i = j - W + e;
+      col[(size_t)j * ND + e] = (i >= 0 && i < n && std::abs(i - j) <= w) ? row[(size_t)i * nd + (j - i + w)] : zc(0, 0);
+    }
+}
+
 int validate(const tdde_config* c, const tdde_c64* S, const tdde_c64* H0, const int32_t* cls, const tdde_term* terms) {
   if (!c || !S || !H0 || !cls) return TDDE_EINVAL;
   if (c->n_ang <= 0 || c->n_rad <= 0 || c->n_cls <= 0 || c->n_cls > c->n_ang) return TDDE_EINVAL;
@@ -96,8 +106,9 @@ bool detect_banded(const tdde_config* c, const tdde_term* terms, int* m0, int* m
 
 extern "C" void tdde_destroy(tdde_handle* h) {
   if (!h) return;
+  DeviceGuard dg(h->device);
   cudaStreamSynchronize(h->stream);
-  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_pslot, h->d_warp_cls, h->d_Wsp, h->d_Corner, h->d_Schur, h->d_rsm, h->d_rsp, h->d_Lcol, h->d_Ucol, h->X, h->r,
+  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_pslot, h->d_warp_cls, h->d_spval, h->d_spcol, h->d_Wsp, h->d_Corner, h->d_Schur, h->d_rsm, h->d_rsp, h->d_Lcol, h->d_Ucol, h->X, h->r,
                   h->rhat, h->p, h->v, h->s, h->t, h->y, h->z, h->c_stage, h->d_st, h->d_st_bench, h->d_partials,
                   h->d_ticket, h->d_g, h->d_g_small, h->d_zero_g};
   for (void* p : ptrs) if (p) cudaFree(p);
@@ -123,39 +134,96 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
   h->nint = (long long)n_rad * h->ld;
   h->n = (long long)c.n_ang * n_rad;
   h->tau = 0.5 * c.dt;
-  h->blk_count = (long long)c.n_cls * n_rad * nd0;
 
+  CU(cudaGetDevice(&h->device));
+  CU(cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device));
   int m0 = 0, ms = 0;
   h->path = detect_banded(&c, terms, &m0, &ms) ? 1 : 0;
+  if (const char* env = std::getenv("TDDE_APPLY_PATH")) { if (std::atoi(env) != 1) h->path = 0; }   // tests: force a lower tier
   h->bT = T; h->bM0 = m0; h->bMS = ms; h->bW = w0;
-  h->norm_banded = (h->path == 1);
   // Term split over two warp groups (256-thread CTA, one per SM, 255 registers each): measured on B200 it wins once
   // the per-thread A_L registers no longer fit (HBM-scale, T = 7: 3.21 -> 2.39 ms) and loses below (Large, T = 5:
   // 0.31 -> 0.37 ms), so it is chosen by the number of terms.
   h->apply_ng = (T >= 6) ? 2 : 1;
   if (const char* env = std::getenv("TDDE_APPLY_NG")) h->apply_ng = std::atoi(env) == 2 ? 2 : 1;
 
-  // radial segment length (banded path): the kernel runs TDDE_AP_MINB CTAs per SM; every segment
-  // recomputes 2 w0 halo rows.  Pick the segment count that minimises waves x (rows + halo).
+  // Staged sparse-A path (tdde_apply_sparse.cu) for everything the register-A kernel does not cover: general sparse A_L
+  // (ELL rows in shared memory), any T, per-term bandwidths padded to one of the instantiated widths.
+  std::vector<zc> ell_val;
+  std::vector<int> ell_col;
+  if (h->path == 0) {
+    int maxw = w0;
+    for (int L = 0; L < T; ++L) maxw = std::max(maxw, (int)terms[L].w);
+    const int widths[4] = {3, 6, 9, 13};
+    int spW = 0;
+    for (int q = 0; q < 4 && !spW; ++q) if (maxw <= widths[q]) spW = widths[q];
+    if (spW) {
+      // ELL rows (duplicate columns of a CSR row summed), the coupling reach, the tile width
+      int nslots = 0, reach = 0;
+      std::vector<std::vector<std::pair<int, zc>>> rows((size_t)T * c.n_ang);
+      for (int L = 0; L < T; ++L) {
+        const zc* val = reinterpret_cast<const zc*>(terms[L].A_val);
+        int mx = 0;
+        for (int a = 0; a < c.n_ang; ++a) {
+          auto& row = rows[(size_t)L * c.n_ang + a];
+          for (int q = terms[L].A_rowptr[a]; q < terms[L].A_rowptr[a + 1]; ++q) {
+            const int col = terms[L].A_col[q];
+            size_t k = 0;
+            while (k < row.size() && row[k].first != col) ++k;
+            if (k == row.size()) row.push_back({col, val[q]}); else row[k].second += val[q];
+            reach = std::max(reach, std::abs(col - a));
+          }
+          mx = std::max(mx, (int)row.size());
+        }
+        h->sp_nslot[L] = mx;
+        nslots += mx;
+      }
+      const bool full = TDDE_AP_NC + 2 * reach >= h->ld;
+      const int xw = full ? h->ld : TDDE_AP_NC + 2 * reach;
+      if (apply_sparse_smem(spW, T, nslots, xw) <= (size_t)220 * 1024 && !std::getenv("TDDE_NO_STAGED")) {
+        h->path = 2; h->spW = spW; h->sp_nslots = nslots; h->sp_xw = xw; h->sp_full = full ? 1 : 0; h->sp_reach = reach;
+        ell_val.assign((size_t)std::max(nslots, 1) * h->ld, zc(0, 0));
+        ell_col.assign((size_t)std::max(nslots, 1) * h->ld, 0);
+        int base = 0;
+        for (int L = 0; L < T; ++L) {
+          for (int a = 0; a < h->ld; ++a)
+            for (int q = 0; q < h->sp_nslot[L]; ++q) {
+              const bool have = a < c.n_ang && q < (int)rows[(size_t)L * c.n_ang + a].size();
+              ell_val[(size_t)(base + q) * h->ld + a] = have ? rows[(size_t)L * c.n_ang + a][q].second : zc(0, 0);
+              ell_col[(size_t)(base + q) * h->ld + a] = have ? rows[(size_t)L * c.n_ang + a][q].first : a;
+            }
+          base += h->sp_nslot[L];
+        }
+      }
+    }
+  }
+  h->norm_banded = (h->path != 0);
+  const int wpad = h->path == 2 ? h->spW : w0;             // half-width of the column bands the apply kernels read
+  const int ndp = 2 * wpad + 1;
+  h->blk_count = (long long)c.n_cls * n_rad * ndp;
+
+  // radial segment length (structured paths): every segment recomputes 2 W halo rows.  Pick the segment count that
+  // minimises waves x (rows + halo) over the resident CTA slots.
   {
     const int chan_blocks = (h->ld + TDDE_AP_NC - 1) / TDDE_AP_NC;
-    const int slots = 148 * (h->apply_ng == 2 ? TDDE_AP_MINB2 : TDDE_AP_MINB);
+    const int per_sm = h->path == 2 ? 1 : (h->apply_ng == 2 ? TDDE_AP_MINB2 : TDDE_AP_MINB);
+    const int slots = h->num_sms * per_sm;
     long long best_cost = -1;
     int best_seg = n_rad;
     for (int segs = 1; segs <= n_rad; ++segs) {
       const int seg = (n_rad + segs - 1) / segs;
-      if (seg < 2 * w0 && segs > 1) break;
+      if (seg < 2 * wpad && segs > 1) break;
       const int real_segs = (n_rad + seg - 1) / seg;
       const long long ctas = (long long)chan_blocks * real_segs;
       const long long waves = (ctas + slots - 1) / slots;
-      const long long cost = waves * (seg + 2 * w0);
+      const long long cost = waves * (seg + 2 * wpad);
       if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_seg = seg; }
     }
     h->seg_len = best_seg;
     // the S-only apply has 13 complex FMAs per element: not ALU-bound, so halo recomputation is cheap and
     // many short segments (about 4 waves of 3 CTAs per SM) hide the TMA latency instead
-    const int want = (4 * 148 * 3 + chan_blocks - 1) / chan_blocks;
-    h->seg_len_s = std::min(n_rad, std::max(4 * w0, (n_rad + want - 1) / want));
+    const int want = (4 * h->num_sms * 3 + chan_blocks - 1) / chan_blocks;
+    h->seg_len_s = h->path == 2 ? h->seg_len : std::min(n_rad, std::max(4 * w0, (n_rad + want - 1) / want));
   }
 
   const zc* S = reinterpret_cast<const zc*>(S_band);
@@ -191,6 +259,7 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
   }
   // block bands S, H0, M+ in the layout of the chosen path; LU of M+
   {
+    const size_t blk_p = (size_t)n_rad * ndp;                // per-class size in the apply kernels' layout
     std::vector<zc> Sx(h->blk_count), Hx(h->blk_count), Mx(h->blk_count);
     std::vector<zc> Lc((size_t)c.n_cls * n_rad * w0), Uc((size_t)c.n_cls * n_rad * (w0 + 1));
     // preconditioner partitions: interiors short enough that a (32 channels x interior) tile plus the factor ring fits
@@ -223,10 +292,10 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
       for (int i = 0; i < n_rad; ++i)
         for (int d = -w0; d <= w0; ++d)
           if (i + d < 0 || i + d >= n_rad) Mrow[(size_t)i * nd0 + d + w0] = zc(0, 0);
-      if (h->path == 1) {
-        row_to_col_band(Sk, &Sx[k * blk_sz], n_rad, w0);
-        row_to_col_band(Hk, &Hx[k * blk_sz], n_rad, w0);
-        row_to_col_band(Mrow.data(), &Mx[k * blk_sz], n_rad, w0);
+      if (h->path != 0) {
+        row_to_col_band_padded(Sk, &Sx[k * blk_p], n_rad, w0, wpad);
+        row_to_col_band_padded(Hk, &Hx[k * blk_p], n_rad, w0, wpad);
+        row_to_col_band_padded(Mrow.data(), &Mx[k * blk_p], n_rad, w0, wpad);
       } else {
         std::memcpy(&Sx[k * blk_sz], Sk, blk_sz * sizeof(zc));
         std::memcpy(&Hx[k * blk_sz], Hk, blk_sz * sizeof(zc));
@@ -240,6 +309,9 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
         return TDDE_ESINGULAR;
       h->lu_growth = std::max(h->lu_growth, growth);
     }
+    // The in-iteration applies of the banded path replace the block part by the known right-hand side of the solve (A y = p + ...),
+    // which is exact up to the backward error of the unpivoted LU, about eps x growth.  Keep that three orders below rtol.
+    h->use_subst = (h->lu_growth * 2.3e-16 <= 1e-3 * c.rtol) && !std::getenv("TDDE_NO_SUBST");
     int rc;
     if ((rc = dev_upload(&h->d_S, reinterpret_cast<cplx*>(Sx.data()), Sx.size(), s))) return rc;
     if ((rc = dev_upload(&h->d_H0, reinterpret_cast<cplx*>(Hx.data()), Hx.size(), s))) return rc;
@@ -295,16 +367,19 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     if ((rc = dev_upload(&h->d_cta_cls, cta_cls.data(), cta_cls.size(), s))) return rc;
     CU(cudaStreamSynchronize(s));
   }
-  if (h->path == 1) {
+  if (h->path != 0) {
     int rc;
-    const int nd = 2 * w0 + 1;
-    std::vector<zc> Rall((size_t)n_rad * std::max(T, 1) * nd), Rc((size_t)n_rad * nd);
+    std::vector<zc> Rall((size_t)n_rad * std::max(T, 1) * ndp), Rc((size_t)n_rad * ndp);
     for (int L = 0; L < T; ++L) {
-      row_to_col_band(reinterpret_cast<const zc*>(terms[L].R_band), Rc.data(), n_rad, w0);
+      row_to_col_band_padded(reinterpret_cast<const zc*>(terms[L].R_band), Rc.data(), n_rad, terms[L].w, wpad);
       for (int j = 0; j < n_rad; ++j)
-        std::memcpy(&Rall[((size_t)j * T + L) * nd], &Rc[(size_t)j * nd], nd * sizeof(zc));
+        std::memcpy(&Rall[((size_t)j * T + L) * ndp], &Rc[(size_t)j * ndp], ndp * sizeof(zc));
     }
     if ((rc = dev_upload(&h->d_Rall, reinterpret_cast<cplx*>(Rall.data()), Rall.size(), s))) return rc;
+    if (h->path == 2) {
+      if ((rc = dev_upload(&h->d_spval, reinterpret_cast<cplx*>(ell_val.data()), ell_val.size(), s))) return rc;
+      if ((rc = dev_upload(&h->d_spcol, ell_col.data(), ell_col.size(), s))) return rc;
+    }
     CU(cudaStreamSynchronize(s));
   }
   for (int L = 0; L < T && h->path == 0; ++L) {

@@ -26,7 +26,7 @@ int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int b
   std::memset(&a, 0, sizeof(a));
   a.x = x; a.y = y; a.aux = aux;
   a.emode = emode; a.oscale = oscale; a.y2 = y2;
-  a.addv = (h->path == 1 && with_terms && h->cfg.n_terms > 0) ? addv : nullptr;
+  a.addv = (h->path == 1 && h->use_subst && with_terms && h->cfg.n_terms > 0) ? addv : nullptr;
   a.n_ang = h->cfg.n_ang; a.n_rad = h->cfg.n_rad; a.ld = h->ld;
   a.seg_len = (with_terms && h->cfg.n_terms > 0) ? h->seg_len : h->seg_len_s;
   a.cls = h->d_cls;
@@ -49,13 +49,21 @@ int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int b
     a.Rall = h->d_Rall; a.slot = h->d_slot; a.cta_cls = h->d_cta_cls;
     a.Aoff = h->d_Aoff;
     rc = launch_apply_banded(a, T, h->bM0, h->bMS, h->cfg.w0, h->apply_ng, h->stream);
+  } else if (h->path == 2) {
+    a.blk = blk_ptr(h, blk);
+    a.Rall = h->d_Rall; a.slot = h->d_slot; a.cta_cls = h->d_cta_cls;
+    a.sp_val = h->d_spval; a.sp_col = h->d_spcol;
+    a.sp_nslots = 0;
+    for (int L = 0; L < T; ++L) { a.sp_nslot[L] = h->sp_nslot[L]; a.sp_nslots += h->sp_nslot[L]; }
+    a.sp_xw = h->sp_xw; a.sp_full = h->sp_full; a.sp_reach = h->sp_reach;
+    rc = launch_apply_sparse(a, h->spW, h->stream);
   } else {
     a.blk_row = blk_ptr(h, blk);
     for (int L = 0; L < T; ++L) {
       a.Rrow[L] = h->d_R[L]; a.w[L] = h->w[L];
       a.A_rowptr[L] = h->d_Arowptr[L]; a.A_col[L] = h->d_Acol[L]; a.A_val[L] = h->d_Aval[L];
     }
-    rc = launch_apply_generic(a, h->stream);
+    rc = launch_apply_generic(a, h->num_sms, h->stream);
   }
   if (rc == -2) return tdde_cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(apply)");
   if (rc < 0) return TDDE_EINVAL;
@@ -233,6 +241,7 @@ static int run_steps(tdde_handle* h, long long n_steps) {
 
 extern "C" int tdde_propagate(tdde_handle* h, tdde_c64* c_dev, int64_t n_steps, const double* g_table, tdde_stats* st) {
   if (!h || !c_dev || n_steps < 0 || (n_steps > 0 && h->cfg.n_terms > 0 && !g_table)) return TDDE_EINVAL;
+  DeviceGuard dg(h->device);
   if (st) std::memset(st, 0, sizeof(*st));
   if (n_steps == 0) return 0;
   int rc;
@@ -255,6 +264,7 @@ extern "C" int tdde_step(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, t
 
 extern "C" int tdde_propagate_host(tdde_handle* h, tdde_c64* c_host, int64_t n_steps, const double* g_table, tdde_stats* st) {
   if (!h || !c_host) return TDDE_EINVAL;
+  DeviceGuard dg(h->device);
   const size_t bytes = (size_t)h->n * sizeof(cplx);
   if (!h->c_stage) CU(cudaMalloc((void**)&h->c_stage, bytes));
   CU(cudaMemcpyAsync(h->c_stage, c_host, bytes, cudaMemcpyHostToDevice, h->stream));
@@ -266,6 +276,7 @@ extern "C" int tdde_propagate_host(tdde_handle* h, tdde_c64* c_host, int64_t n_s
 
 extern "C" int tdde_step_forced(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, int32_t n_iters, tdde_c64* trace_dev) {
   if (!h || !c_dev || n_iters < 0 || (h->cfg.n_terms > 0 && !g_mid)) return TDDE_EINVAL;
+  DeviceGuard dg(h->device);
   int rc;
   if ((rc = upload_g(h, g_mid, 1))) return rc;
   h->h_st->status = 0; h->h_st->stalled = 0; h->h_st->done = 1;
@@ -296,6 +307,7 @@ extern "C" int tdde_step_forced(tdde_handle* h, tdde_c64* c_dev, const double* g
 
 extern "C" int tdde_norm(tdde_handle* h, const tdde_c64* c_dev, double* out) {
   if (!h || !c_dev || !out) return TDDE_EINVAL;
+  DeviceGuard dg(h->device);
   int rc;
   h->launches += launch_to_internal(reinterpret_cast<const cplx*>(c_dev), h->y, h->cfg.n_ang, h->cfg.n_rad, h->ld, h->stream);
   if ((rc = enqueue_apply(h, h->y, h->z, h->y, BLK_S, make_double2(0, 0), false, h->d_zero_g, nullptr, 0, FIN_NORM, h->d_st))) return rc;
@@ -306,6 +318,7 @@ extern "C" int tdde_norm(tdde_handle* h, const tdde_c64* c_dev, double* out) {
 
 extern "C" int tdde_apply(tdde_handle* h, tdde_c64 alpha, tdde_c64 beta, const double* g, const tdde_c64* x_dev, tdde_c64* y_dev) {
   if (!h || !x_dev || !y_dev || x_dev == y_dev || (h->cfg.n_terms > 0 && !g)) return TDDE_EINVAL;
+  DeviceGuard dg(h->device);
   int rc;
   if (h->cfg.n_terms > 0)
     CU(cudaMemcpyAsync(h->d_g_small, g, h->cfg.n_terms * sizeof(double), cudaMemcpyHostToDevice, h->stream));
@@ -320,6 +333,7 @@ extern "C" int tdde_apply(tdde_handle* h, tdde_c64 alpha, tdde_c64 beta, const d
 
 extern "C" int tdde_precond(tdde_handle* h, const tdde_c64* x_dev, tdde_c64* y_dev) {
   if (!h || !x_dev || !y_dev) return TDDE_EINVAL;
+  DeviceGuard dg(h->device);
   int rc;
   h->launches += launch_to_internal(reinterpret_cast<const cplx*>(x_dev), h->y, h->cfg.n_ang, h->cfg.n_rad, h->ld, h->stream);
   if ((rc = enqueue_precond(h, h->y, h->z, nullptr))) return rc;

@@ -18,7 +18,12 @@ struct tdde_handle {
   double tau = 0;                // dt / 2
 
   // apply path
-  int path = 0;                  // 1 banded fast path, 0 generic
+  int path = 0;                  // 1 banded register-A fast path, 2 staged sparse-A path, 0 generic
+  int spW = 0, sp_nslots = 0, sp_xw = 0, sp_full = 0, sp_reach = 0;   // staged sparse-A path
+  int sp_nslot[TDDE_MAX_TERMS] = {};
+  cplx* d_spval = nullptr;
+  int* d_spcol = nullptr;
+  bool use_subst = true;         // banded path: in-iteration applies use A y = p + i tau (coupling) y (needs a benign LU)
   int bT = 0, bM0 = 0, bMS = 0, bW = 0;
   int seg_len = 0;               // radial rows per thread (banded path)
   int seg_len_s = 0;             // radial rows per thread for the S-only (T = 0) apply: latency-bound, wants more CTAs
@@ -72,6 +77,16 @@ struct tdde_handle {
   const double* graph_g = nullptr;
   long long graph_launches = 0;
   bool graph_ok = true;
+};
+
+// Every entry point runs on the device the handle was created on, whatever the caller's current device is.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
 };
 
 extern thread_local std::string g_last_cuda_error;

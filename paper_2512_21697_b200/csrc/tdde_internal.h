@@ -107,6 +107,14 @@ struct ApplyArgs {
   const int* slot;         // [ld] index of the channel's class in its CTA's class list, -1 = not staged
   const int* cta_cls;      // [n_cta][TDDE_AP_MAXC] classes staged per CTA (-1 = unused)
   const cplx* Aoff;        // banded path: [n_slots][ld], slot = (term, offset) in kernel order
+  // staged sparse-A path (tdde_apply_sparse.cu): ELL rows of every term, slot-major [sp_nslots][ld]; blk and Rall padded to 2W+1
+  const cplx* sp_val;
+  const int* sp_col;       // absolute internal channel index (own channel for padding slots)
+  int sp_nslot[TDDE_MAX_TERMS];
+  int sp_nslots;           // sum of sp_nslot
+  int sp_xw;               // channels of the staged x tile
+  int sp_full;             // 1: the tile is the whole row (sp_xw == ld)
+  int sp_reach;            // otherwise: largest |column - row| over all terms; tile = 128 + 2 reach channels
   // generic path
   const int* A_rowptr[TDDE_MAX_TERMS];
   const int* A_col[TDDE_MAX_TERMS];
@@ -155,10 +163,13 @@ struct PrecArgs {
 __host__ __device__ inline int pc_lo(const PrecArgs& p, int q) { return q * (p.int_base + p.w) + (q < p.int_rem ? q : p.int_rem); }
 __host__ __device__ inline int pc_len(const PrecArgs& p, int q) { return p.int_base + (q < p.int_rem ? 1 : 0); }
 
+int tdde_num_sms();   // multiprocessor count of the current device
 // launchers (each returns the number of kernels launched, or -1 if no instantiation fits)
 int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, int ng, cudaStream_t s);
 bool apply_banded_available(int T, int m0, int mstep, int W);
-int launch_apply_generic(const ApplyArgs& a, cudaStream_t s);
+int launch_apply_generic(const ApplyArgs& a, int num_sms, cudaStream_t s);
+int launch_apply_sparse(const ApplyArgs& a, int W, cudaStream_t s);
+size_t apply_sparse_smem(int W, int T, int nslots, int xw);
 int launch_precond(const PrecArgs& a, cudaStream_t s);
 size_t precond_tile_smem(int w, int tile_rows);   // dynamic shared memory of k_precond_tile
 int launch_vec_p(const VecArgs& a, cudaStream_t s);

@@ -23,6 +23,7 @@ extern "C" int tdde_apply_path(const tdde_handle* h) { return h ? h->path : -1; 
 extern "C" int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, const double* g, double* ms_out) {
   if (!h || !ms_out || reps <= 0 || which < 0 || which > 6) return TDDE_EINVAL;
   if (which == 0 && h->cfg.n_terms > 0 && !g) return TDDE_EINVAL;
+  DeviceGuard dg(h->device);
   cudaStream_t s = h->stream;
   SolverState* sb = h->d_st_bench;
   // finite, non-trivial data in every work vector
@@ -68,7 +69,7 @@ extern "C" int tdde_fp64_peak(void* cuda_stream, double* flops_out) {
   cudaStream_t s = (cudaStream_t)cuda_stream;
   double* d = nullptr;
   CU(cudaMalloc((void**)&d, sizeof(double)));
-  const int blocks = 148 * 8, threads = 256, iters = 4096;
+  const int blocks = tdde_num_sms() * 8, threads = 256, iters = 4096;
   launch_dfma_peak(d, blocks, threads, 64, s);
   cudaEvent_t e0, e1;
   CU(cudaEventCreate(&e0));

@@ -132,7 +132,7 @@ extern "C" int tdde_paper_variant(tdde_handle* h, const double* g, const tdde_c6
   PV(cudaMemcpyAsync(d_nch, nch.data(), n_ang * sizeof(int), cudaMemcpyHostToDevice, s));
   PV(cudaMemcpyAsync(d_pref, rad_pref.data(), (n_rad + 1) * sizeof(int), cudaMemcpyHostToDevice, s));
   p.chan_base = d_base; p.nch = d_nch; p.rad_pref = d_pref;
-  const int blocks = 148 * 8;
+  const int blocks = tdde_num_sms() * 8;
   k_pv_rowptr<<<blocks, 256, 0, s>>>(p, n, nnz);
   k_pv_assemble<0><<<blocks, 256, 0, s>>>(p, n);                      // structure: once
   h->launches += 2;

@@ -1,13 +1,25 @@
 // tdde_vec.cu -- fused BiCGSTAB vector kernels (a3 is fused into the start-of-step applies), layout transposes, small helpers.
 //
 // All of these are HBM-bound streaming kernels: 128-bit (double2) coalesced loads/stores, grid-stride over
-// the internal element count, grid = a fixed multiple of the 148 SMs, the inner products fused into the pass
+// the internal element count, grid = a fixed multiple of the SM count, the inner products fused into the pass
 // that produces the vector and finished by the deterministic grid reduction of tdde_reduce.cuh.
 #include "tdde_reduce.cuh"
 
 #define VEC_NT 256
 #define VEC_BLOCKS_PER_SM 8
-#define NUM_SMS 148
+// multiprocessor count of the current device (cached per device)
+int tdde_num_sms() {
+  static int cache[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+  if (cache[dev] == 0) {
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+    cache[dev] = n;
+  }
+  return cache[dev];
+}
+#define NUM_SMS tdde_num_sms()
 
 static int vec_grid(long long n) {
   long long need = (n + VEC_NT - 1) / VEC_NT;

@@ -74,7 +74,7 @@ def hyd():
 def test_paths_selected(tiny, smallmed, hyd):
     assert tiny[1].apply_path == "banded"
     assert smallmed[1].apply_path == "banded"
-    assert hyd[1].apply_path == "generic"
+    assert hyd[1].apply_path == "staged"
 
 
 @pytest.mark.parametrize("which", ["tiny", "smallmed", "hyd"])
@@ -544,4 +544,101 @@ def test_untemplated_bandwidths_and_term_counts(bw, T):
     c = prop.to_device(p.c0)
     st = prop.propagate(c, p.g_table(p.n_steps))
     assert st["steps"] == p.n_steps and rel(c.cpu().numpy(), c_ref) <= 1e-9
+    prop.close()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# The three apply kernels: banded (register A_L), staged (sparse A_L in shared memory), generic (unstaged fall-back)
+def _random_sparse_problem(seed, n_ang, n_r, bandwidths, nnz_row, w0=None, dup=False):
+    """Hermitian-sum coupling with arbitrary sparse (non-banded) A_L, per-term bandwidths, optional duplicate CSR entries."""
+    rng = np.random.default_rng(seed)
+    base = tdde_inputs.make_synthetic(name="sp", n_ang=n_ang, n_r=n_r, bandwidth=2 * (w0 or max(bandwidths)) + 1, n_terms=0, dt=0.004,
+                                      n_steps=3, rtol=1e-10, seed=seed)
+    terms = []
+    for w in bandwidths:
+        dense = np.zeros((n_ang, n_ang), dtype=np.complex128)
+        for a in range(n_ang):
+            cols = rng.choice(n_ang, size=min(nnz_row, n_ang), replace=False)
+            dense[a, cols] += rng.standard_normal(len(cols)) + 1j * rng.standard_normal(len(cols))
+        dense = 0.5 * (dense + dense.conj().T)                      # each term Hermitian (its R_L is, too)
+        rowptr, col, val = [0], [], []
+        for a in range(n_ang):
+            nz = np.nonzero(dense[a])[0]
+            for cc in nz:
+                if dup and rng.random() < 0.3:                        # split one entry into two CSR entries of the same column
+                    col += [cc, cc]; val += [0.25 * dense[a, cc], 0.75 * dense[a, cc]]
+                else:
+                    col.append(cc); val.append(dense[a, cc])
+            rowptr.append(len(col))
+        R = tdde_inputs.synthetic.herm_band(rng, base.n_rad, w)
+        terms.append(tdde_inputs.Term(w=w, R_band=R, A_rowptr=np.asarray(rowptr, np.int32), A_col=np.asarray(col, np.int32),
+                                      A_val=np.asarray(val, np.complex128)))
+    T = len(terms)
+    d = dict(base.__dict__)
+    d.update(terms=terms, g_of_t=lambda t, _T=T: np.full(_T, 0.3 * np.cos(0.057 * t)))
+    return tdde_inputs.Problem(**d)
+
+
+@pytest.mark.parametrize("case", [dict(n_ang=50, n_r=30, bandwidths=[2, 4, 6], nnz_row=3, dup=True),          # per-term widths, duplicates
+                                  dict(n_ang=300, n_r=25, bandwidths=[6, 6, 6], nnz_row=2),                   # wide reach: whole-row x tile
+                                  dict(n_ang=37, n_r=40, bandwidths=[13] * 8, nnz_row=1),                     # hydrogen-like: w = 13, T = 8
+                                  dict(n_ang=200, n_r=20, bandwidths=[3], nnz_row=1, w0=9)])                  # block band wider than the term's
+def test_staged_sparse_apply_path(case):
+    from paper_2512_21697_b200 import Tdde
+    p = _random_sparse_problem(41, **case)
+    prop = Tdde(p)
+    assert prop.apply_path == "staged"
+    ops, fact = orc.assemble(p), orc.factor_precond(p)
+    x = rand_vec(p.n, 8)
+    g = np.linspace(0.4, 1.2, p.n_terms)
+    for alpha, beta in [(1.0, 0.5j * p.dt), (0.3 - 0.2j, 1.0 + 0.5j)]:
+        y = prop.apply(alpha, beta, g, prop.to_device(x)).cpu().numpy()
+        assert rel(y, orc.apply(ops, alpha, beta, g, x)) <= 1e-12, case
+    assert abs(prop.norm(prop.to_device(x)) - orc.s_norm_sq(ops, x)) <= 1e-12 * orc.s_norm_sq(ops, x)
+    c_ref, infos = orc.propagate(p, ops, fact, p.c0, 3)
+    c = prop.to_device(p.c0)
+    st = prop.propagate(c, p.g_table(3))
+    assert st["steps"] == 3 and rel(c.cpu().numpy(), c_ref) <= 1e-9
+    prop.close()
+
+
+def test_generic_fallback_path_and_bounded_grid(monkeypatch):
+    """The unstaged generic kernel (forced here; otherwise only reached for w > 13 or couplings too dense for shared memory):
+    parity, and a shape with more (row, channel-block) work items than reduction slots (70400 > 65536)."""
+    from paper_2512_21697_b200 import Tdde
+    monkeypatch.setenv("TDDE_NO_STAGED", "1")
+    p = _random_sparse_problem(43, n_ang=60, n_r=25, bandwidths=[4, 6], nnz_row=3)
+    prop = Tdde(p)
+    assert prop.apply_path == "generic"
+    ops, fact = orc.assemble(p), orc.factor_precond(p)
+    x = rand_vec(p.n, 2)
+    g = np.array([0.7, -0.4])
+    y = prop.apply(1.0, 0.5j * p.dt, g, prop.to_device(x)).cpu().numpy()
+    assert rel(y, orc.apply(ops, 1.0, 0.5j * p.dt, g, x)) <= 1e-12
+    c_ref, _ = orc.propagate(p, ops, fact, p.c0, 3)
+    c = prop.to_device(p.c0)
+    prop.propagate(c, p.g_table(3))
+    assert rel(c.cpu().numpy(), c_ref) <= 1e-9
+    prop.close()
+    # 16 channel blocks x 4400 rows = 70400 work items; w = 4 is not a banded-kernel width
+    big = tdde_inputs.make_synthetic(name="biggrid", n_ang=2000, n_r=2200, bandwidth=9, n_terms=1, dt=0.002, n_steps=1, rtol=1e-10, seed=5,
+                                     with_c0=False)
+    prop = Tdde(big)
+    assert prop.apply_path == "generic"
+    x = rand_vec(big.n, 4)
+    xd = prop.to_device(x)
+    n_gpu = prop.norm(xd)                                              # S-only apply with the fused grid reduction
+    X = x.reshape(big.n_ang, big.n_rad)
+    ref = 0.0
+    w = big.w0
+    for d in range(-w, w + 1):
+        lo, hi = max(0, -d), min(big.n_rad, big.n_rad - d)
+        ref += float(np.real(np.sum(np.conj(X[:, lo:hi]) * (0.3 ** abs(d)) * X[:, lo + d:hi + d])))
+    assert abs(n_gpu - ref) <= 1e-11 * ref
+    g = np.array([0.9])
+    y = prop.apply(1.0, 0.5j * big.dt, g, xd).cpu().numpy().reshape(big.n_ang, big.n_rad)
+    rng = np.random.default_rng(0)
+    chan, rad = rng.integers(0, big.n_ang, 200), rng.integers(0, big.n_rad, 200)
+    refs = orc.apply_rows_sampled(big, 1.0, 0.5j * big.dt, g, x, chan, rad)
+    assert np.max(np.abs(y[chan, rad] - refs)) <= 1e-12 * np.sqrt(np.mean(np.abs(refs) ** 2))
     prop.close()
