@@ -27,11 +27,42 @@ import tdde_inputs  # noqa: E402
 
 METRIC = "cn_time_steps_per_s"
 UNIT = "steps/s"
-NUM_SMS = 148
-# dram__bytes_read.sum + dram__bytes_write.sum of one operator-apply launch, from one `ncu --set full` capture
-# (profiles/r01_apply_hbm_ncu.txt); bench.py cannot run ncu itself, so other configs report null
-MEASURED_DRAM_BYTES_PER_APPLY = {"hbm": 2.062e9}
 FP64_FMA_PER_CLK_PER_SM = 64          # B200: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2 TFLOP/s nominal
+WORKLOADS = sorted(tdde_inputs.CONFIGS) + ["hydrogen"]
+# dram__bytes_read.sum + dram__bytes_write.sum of one in-iteration operator-apply launch per workload, from `ncu --set full`
+# captures; bench.py cannot run ncu itself, so it reads the table kept beside the captures (profiles/r02_apply_traffic.md
+# names the command).  A workload without a row reports null.
+TRAFFIC_TABLE = os.path.join(ROOT, "profiles", "r02_apply_traffic.csv")
+
+
+def load_problem(name: str, phase: float = 0.0, e0=None, **kw):
+    """BASELINE.json configs by name; "hydrogen" = configs[1] with the 1s1/2 state as c0 and the pulse shifted to its maximum."""
+    if name == "hydrogen":
+        import scipy.linalg as sla
+        p = tdde_inputs.make_hydrogen(**({} if e0 is None else {"e0": e0}))
+        S, H = p.meta["dense"][-1]
+        E, V = sla.eigh(H, S)
+        j = int(np.nonzero(E > -p.meta["c"] ** 2)[0][0])
+        a = p.meta["chans"].index((-1, 0.5))
+        p.c0[a * p.n_rad:(a + 1) * p.n_rad] = V[:, j]
+        return p
+    if e0 is not None:
+        kw["e0"] = e0
+    return tdde_inputs.make_config(name, phase=phase, **kw)
+
+
+def measured_traffic(workload: str):
+    if not os.path.exists(TRAFFIC_TABLE):
+        return None
+    with open(TRAFFIC_TABLE) as f:
+        for line in f:
+            cells = [c.strip() for c in line.split(",")]
+            if len(cells) >= 2 and cells[0] == workload:
+                try:
+                    return float(cells[1])
+                except ValueError:
+                    return None
+    return None
 
 
 def f_apply(p) -> int:
@@ -42,6 +73,11 @@ def f_apply(p) -> int:
         nnz_row = int(np.max(np.diff(t.A_rowptr)))       # interior rows
         tot += (2 * t.w + 1) + nnz_row
     return tot
+
+
+def num_sms() -> int:
+    import torch
+    return int(torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count)
 
 
 def load_peaks():
@@ -94,46 +130,74 @@ class ClockSampler(threading.Thread):
 
 
 # ----------------------------------------------------------------------------------------------- reference arm
-def oracle_sample_problem(cfg_name: str, sample_ang: int):
+FULL_CSR_MAX_N = 600_000        # the oracle's explicit CSR fits comfortably (Medium: 0.2 G non-zeros)
+FULL_PANELS_MAX_N = 8_000_000   # the oracle's matrix-free form on the WHOLE config stays near 20 s per step (Large)
+
+
+def oracle_sample_problem(cfg_name: str, sample_ang: int, phase: float, e0):
     """The same workload recipe restricted to `sample_ang` angular channels (all radial sizes, bandwidth, terms kept)."""
     args = dict(tdde_inputs.CONFIGS[cfg_name])
     full_n = args["n_ang"] * 2 * args["n_r"]
     args["n_ang"] = min(sample_ang, args["n_ang"])
-    p = tdde_inputs.make_synthetic(name=cfg_name + "-sample", **args)
+    if e0 is not None:
+        args["e0"] = e0
+    p = tdde_inputs.make_synthetic(name=cfg_name + "-sample", phase=phase, **args)
     return p, full_n
 
 
-def run_oracle(cfg_name: str, steps: int, warmup: int, sample_ang: int):
-    """Times the CPU oracle as it stands (SciPy CSR + textbook BiCGSTAB, one thread) on a bounded sample."""
+def run_oracle(cfg_name: str, steps: int, warmup: int, sample_ang: int, phase: float = 0.0, e0=None, allow_panels: bool = True):
+    """Times the CPU oracle as it stands (SciPy CSR / NumPy + textbook BiCGSTAB, one thread).
+    Small workloads (Tiny, Hydrogen, Medium) run WHOLE: a measured number.  Large runs whole through the oracle's
+    matrix-free form (also measured).  HBM-scale would need minutes per step: there the recipe is cut to `sample_ang`
+    channels and the rate is scaled by n_sample / n_full -- labelled "extrapolated"."""
     from oracle import tdde_oracle as orc
-    p, full_n = oracle_sample_problem(cfg_name, sample_ang)
-    ops = orc.assemble(p)
-    fact = orc.factor_precond(p)
+    n_full = None if cfg_name == "hydrogen" else tdde_inputs.CONFIGS[cfg_name]["n_ang"] * 2 * tdde_inputs.CONFIGS[cfg_name]["n_r"]
+    extrapolated, mode = False, "whole workload, explicit CSR"
+    if cfg_name == "hydrogen" or n_full <= FULL_CSR_MAX_N:
+        p = load_problem(cfg_name, phase, e0)
+        full_n = p.n
+        ops = orc.assemble(p)
+        fact = orc.factor_precond(p)
+        step = lambda c, s: orc.cn_step(ops, fact, c, p.g_mid(s), p.dt, p.rtol, p.max_iter, assembled=False)
+    elif n_full <= FULL_PANELS_MAX_N and allow_panels:
+        p = load_problem(cfg_name, phase, e0)
+        full_n = p.n
+        fact = orc.factor_precond(p)
+        mode = "whole workload, matrix-free panels (CSR would need ~25 GB)"
+        step = lambda c, s: orc.cn_step_panels(p, fact, c, p.g_mid(s), p.dt, p.rtol, p.max_iter)
+    else:
+        p, full_n = oracle_sample_problem(cfg_name, sample_ang, phase, e0)
+        ops = orc.assemble(p)
+        fact = orc.factor_precond(p)
+        extrapolated = True
+        mode = (f"recipe cut to {p.n_ang} of {tdde_inputs.CONFIGS[cfg_name]['n_ang']} angular channels (n={p.n}); "
+                "value = sample steps/s x n_sample/n_full")
+        step = lambda c, s: orc.cn_step(ops, fact, c, p.g_mid(s), p.dt, p.rtol, p.max_iter)
     c = p.c0.copy()
-    if warmup:
-        c, _ = orc.propagate(p, ops, fact, c, warmup, first_step=0)
+    for s_ in range(warmup):
+        c, _ = step(c, s_)
+    half = 0
     t0 = time.perf_counter()
-    c, infos = orc.propagate(p, ops, fact, c, steps, first_step=warmup)
+    for s_ in range(steps):
+        c, info = step(c, warmup + s_)
+        half += info.half_iters
     dt = time.perf_counter() - t0
-    sample_steps_per_s = steps / dt
-    scaled = sample_steps_per_s * p.n / full_n
-    return dict(value=scaled, unit=UNIT, cores=1, kind="oracle",
-                sample=f"{cfg_name} recipe cut to {p.n_ang} of {tdde_inputs.CONFIGS[cfg_name]['n_ang']} angular channels "
-                       f"(n={p.n}), {steps} CN steps in {dt:.2f} s; value = sample steps/s x n_sample/n_full",
-                half_iters=int(sum(i.half_iters for i in infos)), seconds=dt), p
+    value = steps / dt * (p.n / full_n)
+    return dict(value=value, unit=UNIT, cores=1, kind="oracle", extrapolated=extrapolated, steps=steps, seconds=dt, half_iters=half,
+                sample=f"{cfg_name}: {mode}; {steps} CN steps in {dt:.2f} s on 1 core"), p
 
 
 def reference_main(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    steps = max(1, min(args.steps, 4))
-    cb, p = run_oracle(args.config, steps, min(args.warmup, 1), args.sample_ang)
+    # every timed step is a bounded sample of the workload (whole for the small configs, a channel cut for Large / HBM-scale)
+    cb, p = run_oracle(args.config, args.steps, args.warmup, args.sample_ang, args.phase, args.e0, allow_panels=False)
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / cb["value"], "higher_is_better": True,
+            "steps": cb["steps"], "warmup": args.warmup, "ms_per_step": 1e3 / cb["value"], "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.config, "note": "CPU oracle on a bounded sample, scaled to the full workload"},
-            "cpu_baseline": {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "config": {"workload": args.config, "phase": args.phase, "note": "CPU oracle: " + cb["sample"]},
+            "cpu_baseline": {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample", "extrapolated")},
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -170,7 +234,7 @@ def ours_main(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     K, W = args.steps, max(args.warmup, 3)
-    p = tdde_inputs.make_config(args.config, phase=args.phase)
+    p = load_problem(args.config, args.phase, args.e0)
     prop = Tdde(p, device=f"cuda:{local}")
     g_all = p.g_table(W + K)
     c = prop.to_device(p.c0)
@@ -197,7 +261,7 @@ def ours_main(args):
     norm_end = prop.norm(c)
 
     # ---- per-kernel timings, live, CUDA events on the handle's stream (same process, right after) ----
-    g_mid = g_all[W]
+    g_mid = np.where(g_all[W] == 0.0, 1e-3, g_all[W])          # per-kernel timings: never a field that is exactly zero
     reps = args.kernel_reps
     kt = {name: prop.time_kernel(which, reps, g_mid) for which, name in
           [(0, "apply"), (1, "precond"), (2, "vec_p"), (3, "vec_s"), (4, "vec_xr"), (5, "transpose"), (6, "apply_S")]}
@@ -221,23 +285,34 @@ def ours_main(args):
     prop.propagate_host(c_host, g_all[W:W + K], K)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
+    # the same K steps as K calls of one step each: the state crosses PCIe both ways on EVERY step
+    c_host[:] = p.c0
+    prop.propagate_host(c_host, g_all[:W], W)
+    barrier()
+    t0 = time.perf_counter()
+    for s_ in range(K):
+        prop.propagate_host(c_host, g_all[W + s_:W + s_ + 1], 1)
+    torch.cuda.synchronize()
+    e2e1_s = time.perf_counter() - t0
 
-    ms, e2e_ms = max_over_ranks([ms, e2e_s * 1e3], device="cuda")
+    ms, e2e_ms, e2e1_ms = max_over_ranks([ms, e2e_s * 1e3, e2e1_s * 1e3], device="cuda")
 
     if rank == 0:
         peaks, peak_kind = load_peaks()
         # the timed kernel is the in-iteration apply v = p + i tau (coupling terms) y: the block part (n_d cFMA) is replaced
         # by adding the known vector p, so it is not counted
-        F = f_apply(p) - (2 * p.w0 + 1) if prop.apply_path == "banded" else f_apply(p)
+        subst = prop.apply_path == "banded" and T > 0
+        F = f_apply(p) - (2 * p.w0 + 1) if subst else f_apply(p)
         nint = n                                            # algorithmic element count (pads excluded)
         flops_apply = 8.0 * F * nint
         sm_max = float(peaks.get("sm_max_mhz", 1965.0))
-        fp64_peak_nominal = NUM_SMS * FP64_FMA_PER_CLK_PER_SM * 2 * sm_max * 1e6
-        traffic = MEASURED_DRAM_BYTES_PER_APPLY.get(args.config)
+        n_sm = num_sms()
+        fp64_peak_nominal = n_sm * FP64_FMA_PER_CLK_PER_SM * 2 * sm_max * 1e6
+        traffic = measured_traffic(args.config)
         t_apply = kt["apply"] * 1e-3
         ach = flops_apply / t_apply / 1e12
         hbm = float(peaks["hbm_gbs"])
-        bytes_per = {"apply": 64 if prop.apply_path == "banded" else 48, "precond": 32, "vec_p": 64, "vec_s": 48, "vec_xr": 128, "transpose": 32, "apply_S": 32}
+        bytes_per = {"apply": 64 if subst else 48, "precond": 32, "vec_p": 64, "vec_s": 48, "vec_xr": 128, "transpose": 32, "apply_S": 32}
         kernels = {k: {"ms": v, "alg_GBps": bytes_per[k] * nint / (v * 1e-3) / 1e9,
                        "hbm_frac": bytes_per[k] * nint / (v * 1e-3) / 1e9 / hbm} for k, v in kt.items()}
         steps_per_s = whole_job_rate(world, K, ms)
@@ -246,7 +321,7 @@ def ours_main(args):
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.config, "n_ang": p.n_ang, "n_rad": p.n_rad, "n": n, "bandwidth": 2 * p.w0 + 1,
-                       "n_terms": T, "dt": p.dt, "rtol": p.rtol, "seed": p.seed, "phase": args.phase,
+                       "n_terms": T, "dt": p.dt, "rtol": p.rtol, "seed": p.seed, "phase": args.phase, "e0": p.meta.get("e0"),
                        "apply_path": prop.apply_path, "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "vectors (%.0f MB each) exceed the 126 MB L2; no flush" % (n * 16 / 1e6)},
             "bicgstab_iters_per_s": world * 0.5 * st["half_iters"] / (ms * 1e-3),
@@ -256,12 +331,17 @@ def ours_main(args):
             "clocks": clocks,
             "e2e": {"value": whole_job_rate(world, K, e2e_ms), "unit": UNIT,
                     "h2d_bytes_per_step": (n * 16 + K * T * 8) / K, "d2h_bytes_per_step": n * 16 / K,
-                    "note": "one tdde_propagate_host call of K steps: state vector H2D + g table H2D + K steps + state D2H"},
-            "roofline": {"bound": "alu", "kernel": "k_apply_banded (v = A y = p + i tau (sum_L g_L A_L (x) R_L) y with fused <rhat,v>)",
+                    "note": "one tdde_propagate_host call of K steps: state vector H2D + g table H2D + K steps + state D2H",
+                    "per_step_copies": {"value": whole_job_rate(world, K, e2e1_ms), "unit": UNIT,
+                                        "h2d_bytes_per_step": n * 16 + T * 8, "d2h_bytes_per_step": n * 16,
+                                        "note": "K tdde_propagate_host calls of one step each"}},
+            "roofline": {"bound": "alu",
+                         "kernel": ("k_apply_banded (v = A y = p + i tau (sum_L g_L A_L (x) R_L) y with fused <rhat,v>)" if subst else
+                                    "k_apply_%s (v = A y with fused <rhat,v>)" % ("sparse" if prop.apply_path == "staged" else prop.apply_path)),
                          "achieved": ach, "peak": fp64_peak_nominal / 1e12, "unit": "TFLOP/s",
                          "frac": ach / (fp64_peak_nominal / 1e12), "traffic": traffic,
                          "algorithmic_bytes_per_launch": bytes_per["apply"] * nint,
-                         "peak_kind": "derived: 148 SMs x 64 DFMA/clk x 2 x %.0f MHz" % sm_max,
+                         "peak_kind": "derived: %d SMs x 64 DFMA/clk x 2 x %.0f MHz" % (n_sm, sm_max),
                          "fp64_peak_measured_tflops": fp64_peak_meas / 1e12,
                          "frac_of_measured_dfma": ach / (fp64_peak_meas / 1e12),
                          "cfma_per_element": F, "flops_per_launch": flops_apply,
@@ -270,8 +350,9 @@ def ours_main(args):
             "paper_variant": pv,
         }
         if world == 1 and not args.no_cpu_baseline:
-            cb, _ = run_oracle(args.config, 4, 0, args.sample_ang)
-            line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+            n_o = 1 if p.n > FULL_CSR_MAX_N and p.n <= FULL_PANELS_MAX_N else 4
+            cb, _ = run_oracle(args.config, n_o, 0, args.sample_ang, args.phase, args.e0)
+            line["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample", "extrapolated")}
         print(json.dumps(line))
     prop.close()
     if world > 1:
@@ -284,8 +365,10 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="hbm", choices=sorted(tdde_inputs.CONFIGS))
+    ap.add_argument("--config", default="hbm", choices=WORKLOADS)
     ap.add_argument("--phase", type=float, default=0.0, help="phase of g(t) = E0 sin(w t + phase); 0 = BASELINE config")
+    ap.add_argument("--e0", type=float, default=None, help="field amplitude E0 (default: the BASELINE value 0.05); the supplementary "
+                    "stress run of SURVEY 8(d) D2 uses --phase 1.5708 with a larger E0 so that a step needs several full iterations")
     ap.add_argument("--kernel-reps", type=int, default=10)
     ap.add_argument("--sample-ang", type=int, default=24, help="angular channels of the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
