@@ -28,7 +28,7 @@ import tdde_inputs  # noqa: E402
 METRIC = "cn_time_steps_per_s"
 UNIT = "steps/s"
 FP64_FMA_PER_CLK_PER_SM = 64          # B200: 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2 TFLOP/s nominal
-WORKLOADS = sorted(tdde_inputs.CONFIGS) + ["hydrogen"]
+WORKLOADS = sorted(tdde_inputs.CONFIGS) + ["hydrogen", "nondipole"]
 # dram__bytes_read.sum + dram__bytes_write.sum of one in-iteration operator-apply launch per workload, from `ncu --set full`
 # captures; bench.py cannot run ncu itself, so it reads the table kept beside the captures (profiles/r02_apply_traffic.md
 # names the command).  A workload without a row reports null.
@@ -46,6 +46,10 @@ def load_problem(name: str, phase: float = 0.0, e0=None, **kw):
         a = p.meta["chans"].index((-1, 0.5))
         p.c0[a * p.n_rad:(a + 1) * p.n_rad] = V[:, j]
         return p
+    if name == "nondipole":       # x-polarised non-dipole operator set, kappa_max = 15, l_max = 2 (24 terms)
+        from tdde_inputs import nondipole as nd
+        return nd.set_ground_state(nd.make_nondipole(kappa_max=15, l_max=2, n_r=100, r_max=60.0, t_offset=6.0,
+                                                     **({} if e0 is None else {"e0": e0})))
     if e0 is not None:
         kw["e0"] = e0
     return tdde_inputs.make_config(name, phase=phase, **kw)
@@ -151,9 +155,16 @@ def run_oracle(cfg_name: str, steps: int, warmup: int, sample_ang: int, phase: f
     matrix-free form (also measured).  HBM-scale would need minutes per step: there the recipe is cut to `sample_ang`
     channels and the rate is scaled by n_sample / n_full -- labelled "extrapolated"."""
     from oracle import tdde_oracle as orc
-    n_full = None if cfg_name == "hydrogen" else tdde_inputs.CONFIGS[cfg_name]["n_ang"] * 2 * tdde_inputs.CONFIGS[cfg_name]["n_r"]
+    special = cfg_name in ("hydrogen", "nondipole")
+    n_full = None if special else tdde_inputs.CONFIGS[cfg_name]["n_ang"] * 2 * tdde_inputs.CONFIGS[cfg_name]["n_r"]
     extrapolated, mode = False, "whole workload, explicit CSR"
-    if cfg_name == "hydrogen" or n_full <= FULL_CSR_MAX_N:
+    if cfg_name == "nondipole":
+        p = load_problem(cfg_name, phase, e0)
+        full_n = p.n
+        fact = orc.factor_precond(p)
+        mode = "whole workload, matrix-free panels"
+        step = lambda c, s: orc.cn_step_panels(p, fact, c, p.g_mid(s), p.dt, p.rtol, p.max_iter)
+    elif cfg_name == "hydrogen" or n_full <= FULL_CSR_MAX_N:
         p = load_problem(cfg_name, phase, e0)
         full_n = p.n
         ops = orc.assemble(p)

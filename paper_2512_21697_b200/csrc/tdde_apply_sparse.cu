@@ -8,7 +8,8 @@
 // couple to), the radial column coefficients of all terms and the block coefficients of the CTA's kappa-classes arrive by 1-D
 // TMA bulk copies in a two-stage mbarrier ring.  What differs: A_L is an arbitrary sparse matrix, any number of terms up to
 // TDDE_MAX_TERMS, per-term bandwidths up to W.  The rows of A_L (ELL: values pre-multiplied by beta g_L, column positions
-// relative to the x tile) live in SHARED memory, one column per thread, loaded once per CTA; the angular combination
+// absolute channel index) live in SHARED memory, one column per thread, loaded once per CTA, when they fit, and are otherwise read
+// from global memory (L1/L2) once per input row; the angular combination
 // z_L = sum_q A_L[a', q] x[col_q] is formed per input row and pushed through the radial band from warp-broadcast coefficients.
 #include "tdde_reduce.cuh"
 
@@ -46,8 +47,9 @@ __host__ __device__ inline size_t sparse_stage_elems(int W, int T, int xw) {
   const int ND = 2 * W + 1;
   return (size_t)SP_JC * T * ND + (size_t)SP_MAXC * SP_JC * ND + (size_t)SP_JC * xw;
 }
-size_t apply_sparse_smem(int W, int T, int nslots, int xw) {
-  return (size_t)nslots * SP_NC * (sizeof(cplx) + sizeof(int)) + SP_NST * sparse_stage_elems(W, T, xw) * sizeof(cplx) + 64;
+size_t apply_sparse_smem(int W, int T, int nslots, int xw, bool a_in_smem) {
+  return (a_in_smem ? (size_t)nslots * SP_NC * (sizeof(cplx) + sizeof(int)) : 0) + SP_NST * sparse_stage_elems(W, T, xw) * sizeof(cplx) +
+         TDDE_MAX_TERMS * sizeof(cplx) + 64;
 }
 
 template <int W>
@@ -61,9 +63,11 @@ __global__ void __launch_bounds__(SP_NC, 1) k_apply_sparse(const __grid_constant
   const size_t stage = sparse_stage_elems(W, T, XW);
   const int RS = JC * T * ND, BS = SP_MAXC * JC * ND;
   cplx* stage_base = reinterpret_cast<cplx*>(smem_raw);
-  cplx* Av = stage_base + SP_NST * stage;                    // [S][128]
-  int* Ac = reinterpret_cast<int*>(Av + (size_t)S * SP_NC);  // [S][128]
-  uint64_t* full = reinterpret_cast<uint64_t*>(Ac + (size_t)S * SP_NC);          // S * 128 ints: 8-byte aligned
+  cplx* coefL = stage_base + SP_NST * stage;                 // [TDDE_MAX_TERMS] beta g_L
+  cplx* Av_s = coefL + TDDE_MAX_TERMS;                       // [S][128] (only when sp_a_smem)
+  const size_t Sa = p.sp_a_smem ? (size_t)S : 0;
+  int* Ac_s = reinterpret_cast<int*>(Av_s + Sa * SP_NC);     // [S][128]
+  uint64_t* full = reinterpret_cast<uint64_t*>(Ac_s + Sa * SP_NC);               // S * 128 ints: 8-byte aligned
 
   const int tid = threadIdx.x, ld = p.ld, n_rad = p.n_rad;
   const int a0 = blockIdx.x * SP_NC, a = a0 + tid;
@@ -83,19 +87,21 @@ __global__ void __launch_bounds__(SP_NC, 1) k_apply_sparse(const __grid_constant
   const int* cta_cls = p.cta_cls + blockIdx.x * SP_MAXC;
 
   for (size_t q = tid; q < SP_NST * stage; q += SP_NC) stage_base[q] = make_double2(0, 0);
-  // rows of A_L for this thread's channel, pre-multiplied by beta g_L (own column of the shared arrays: no hazard)
-  {
+  // rows of A_L for this thread's channel: copied to shared memory when they fit (own column of the shared arrays: no hazard),
+  // otherwise read from global memory per row; the factor beta g_L is applied to z_L
+  if (tid < T) {
     const double* g = p.g + (p.step_ptr ? (size_t)(*p.step_ptr) * T : 0);
-    int s = 0;
-    for (int L = 0; L < T; ++L) {
-      const double gl = g[L];
-      const cplx coef = make_double2(p.beta.x * gl, p.beta.y * gl);
-      for (int q = 0; q < p.sp_nslot[L]; ++q, ++s) {
-        Av[(size_t)s * SP_NC + tid] = cmul(coef, p.sp_val[(size_t)s * ld + ac]);
-        Ac[(size_t)s * SP_NC + tid] = p.sp_col[(size_t)s * ld + ac] - win_lo;
-      }
+    coefL[tid] = make_double2(p.beta.x * g[tid], p.beta.y * g[tid]);
+  }
+  if (p.sp_a_smem) {
+    for (int s = 0; s < S; ++s) {
+      Av_s[(size_t)s * SP_NC + tid] = p.sp_val[(size_t)s * ld + ac];
+      Ac_s[(size_t)s * SP_NC + tid] = p.sp_col[(size_t)s * ld + ac];
     }
   }
+  const cplx* Av = p.sp_a_smem ? Av_s + tid : p.sp_val + ac;
+  const int* Ac = p.sp_a_smem ? Ac_s + tid : p.sp_col + ac;
+  const size_t astr = p.sp_a_smem ? SP_NC : ld;
   if (tid == 0) {
     for (int q = 0; q < SP_NST; ++q) mbar_init(&full[q], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -154,17 +160,18 @@ __global__ void __launch_bounds__(SP_NC, 1) k_apply_sparse(const __grid_constant
           for (int e = 0; e < ND; ++e) cfma(yw[e], __ldg(bc + e), x0);
         }
         int s = 0;
+        const cplx* xw0 = xs - win_lo;                        // absolute channel index -> tile column
 #pragma unroll 1
         for (int L = 0; L < T; ++L) {
           cplx z0 = make_double2(0, 0), z1 = make_double2(0, 0);
           const int ns = p.sp_nslot[L];
           int q = 0;
           for (; q + 1 < ns; q += 2, s += 2) {
-            cfma(z0, Av[(size_t)s * SP_NC + tid], xs[Ac[(size_t)s * SP_NC + tid]]);
-            cfma(z1, Av[(size_t)(s + 1) * SP_NC + tid], xs[Ac[(size_t)(s + 1) * SP_NC + tid]]);
+            cfma(z0, Av[(size_t)s * astr], xw0[Ac[(size_t)s * astr]]);
+            cfma(z1, Av[(size_t)(s + 1) * astr], xw0[Ac[(size_t)(s + 1) * astr]]);
           }
-          if (q < ns) { cfma(z0, Av[(size_t)s * SP_NC + tid], xs[Ac[(size_t)s * SP_NC + tid]]); ++s; }
-          const cplx z = cadd(z0, z1);
+          if (q < ns) { cfma(z0, Av[(size_t)s * astr], xw0[Ac[(size_t)s * astr]]); ++s; }
+          const cplx z = cmul(coefL[L], cadd(z0, z1));
           const cplx* rc = st + ((size_t)r * T + L) * ND;    // warp-uniform: broadcast LDS.128
 #pragma unroll
           for (int e = 0; e < ND; ++e) cfma(yw[e], rc[e], z);
@@ -194,7 +201,7 @@ __global__ void __launch_bounds__(SP_NC, 1) k_apply_sparse(const __grid_constant
 
 int launch_apply_sparse(const ApplyArgs& a, int W, cudaStream_t s) {
   dim3 grid((a.ld + SP_NC - 1) / SP_NC, (a.n_rad + a.seg_len - 1) / a.seg_len);
-  const size_t smem = apply_sparse_smem(W, a.n_terms, a.sp_nslots, a.sp_xw);
+  const size_t smem = apply_sparse_smem(W, a.n_terms, a.sp_nslots, a.sp_xw, a.sp_a_smem != 0);
 #define X(w)                                                                                                           \
   if (W == w) {                                                                                                        \
     if (cudaFuncSetAttribute(k_apply_sparse<w>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -2; \

@@ -180,8 +180,10 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
       }
       const bool full = TDDE_AP_NC + 2 * reach >= h->ld;
       const int xw = full ? h->ld : TDDE_AP_NC + 2 * reach;
-      if (apply_sparse_smem(spW, T, nslots, xw) <= (size_t)220 * 1024 && !std::getenv("TDDE_NO_STAGED")) {
-        h->path = 2; h->spW = spW; h->sp_nslots = nslots; h->sp_xw = xw; h->sp_full = full ? 1 : 0; h->sp_reach = reach;
+      const size_t cap = (size_t)220 * 1024;
+      const bool a_smem = apply_sparse_smem(spW, T, nslots, xw, true) <= cap && !std::getenv("TDDE_SPARSE_A_GLOBAL");
+      if ((a_smem || apply_sparse_smem(spW, T, nslots, xw, false) <= cap) && !std::getenv("TDDE_NO_STAGED")) {
+        h->path = 2; h->spW = spW; h->sp_a_smem = a_smem ? 1 : 0; h->sp_nslots = nslots; h->sp_xw = xw; h->sp_full = full ? 1 : 0; h->sp_reach = reach;
         ell_val.assign((size_t)std::max(nslots, 1) * h->ld, zc(0, 0));
         ell_col.assign((size_t)std::max(nslots, 1) * h->ld, 0);
         int base = 0;

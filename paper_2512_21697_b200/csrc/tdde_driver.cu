@@ -55,7 +55,7 @@ int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int b
     a.sp_val = h->d_spval; a.sp_col = h->d_spcol;
     a.sp_nslots = 0;
     for (int L = 0; L < T; ++L) { a.sp_nslot[L] = h->sp_nslot[L]; a.sp_nslots += h->sp_nslot[L]; }
-    a.sp_xw = h->sp_xw; a.sp_full = h->sp_full; a.sp_reach = h->sp_reach;
+    a.sp_xw = h->sp_xw; a.sp_full = h->sp_full; a.sp_reach = h->sp_reach; a.sp_a_smem = h->sp_a_smem;
     rc = launch_apply_sparse(a, h->spW, h->stream);
   } else {
     a.blk_row = blk_ptr(h, blk);

@@ -19,7 +19,7 @@ struct tdde_handle {
 
   // apply path
   int path = 0;                  // 1 banded register-A fast path, 2 staged sparse-A path, 0 generic
-  int spW = 0, sp_nslots = 0, sp_xw = 0, sp_full = 0, sp_reach = 0;   // staged sparse-A path
+  int spW = 0, sp_nslots = 0, sp_xw = 0, sp_full = 0, sp_reach = 0, sp_a_smem = 1;   // staged sparse-A path
   int sp_nslot[TDDE_MAX_TERMS] = {};
   cplx* d_spval = nullptr;
   int* d_spcol = nullptr;

@@ -11,7 +11,7 @@
 #include <stdint.h>
 #include "tdde.h"
 
-#define TDDE_MAX_TERMS 8
+#define TDDE_MAX_TERMS 24
 #define TDDE_MAX_PARTIAL_BLOCKS 65536
 #define TDDE_TINY 1e-290
 #ifndef TDDE_AP_NC
@@ -115,6 +115,7 @@ struct ApplyArgs {
   int sp_xw;               // channels of the staged x tile
   int sp_full;             // 1: the tile is the whole row (sp_xw == ld)
   int sp_reach;            // otherwise: largest |column - row| over all terms; tile = 128 + 2 reach channels
+  int sp_a_smem;           // 1: the ELL rows of the CTA's channels are copied to shared memory once; 0: read from global (L1/L2) per row
   // generic path
   const int* A_rowptr[TDDE_MAX_TERMS];
   const int* A_col[TDDE_MAX_TERMS];
@@ -169,7 +170,7 @@ int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, int
 bool apply_banded_available(int T, int m0, int mstep, int W);
 int launch_apply_generic(const ApplyArgs& a, int num_sms, cudaStream_t s);
 int launch_apply_sparse(const ApplyArgs& a, int W, cudaStream_t s);
-size_t apply_sparse_smem(int W, int T, int nslots, int xw);
+size_t apply_sparse_smem(int W, int T, int nslots, int xw, bool a_in_smem);
 int launch_precond(const PrecArgs& a, cudaStream_t s);
 size_t precond_tile_smem(int w, int tile_rows);   // dynamic shared memory of k_precond_tile
 int launch_vec_p(const VecArgs& a, cudaStream_t s);

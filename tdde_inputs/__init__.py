@@ -11,3 +11,4 @@ Recipes: DESIGN.md section "Inputs"; SURVEY.md section 8(d) D2 (synthetic) and
 from .problem import Problem, Term, band_to_dense, dense_to_band  # noqa: F401
 from .synthetic import make_synthetic, CONFIGS, make_config  # noqa: F401
 from .hydrogen import make_hydrogen  # noqa: F401
+from .nondipole import make_nondipole  # noqa: F401

@@ -642,3 +642,56 @@ def test_generic_fallback_path_and_bounded_grid(monkeypatch):
     refs = orc.apply_rows_sampled(big, 1.0, 0.5j * big.dt, g, x, chan, rad)
     assert np.max(np.abs(y[chan, rad] - refs)) <= 1e-12 * np.sqrt(np.mean(np.abs(refs) ** 2))
     prop.close()
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# NEXT-1: the paper-shaped non-dipole operator set (x-polarised, mu' = mu +- 1, l <= l_max, 8 Kronecker terms per l)
+def test_nondipole_operator_set_parity():
+    """Eq. 17-18 of the paper (H^theta_l from Clebsch-Gordan x 3j, 24 Kronecker terms for l_max = 2, real Dirac DKB blocks,
+    seeded stand-ins for the radial g^n_l): apply <= 1e-12 and propagation <= 1e-9 against the oracle, on the staged sparse-A kernel."""
+    from paper_2512_21697_b200 import Tdde
+    from tdde_inputs import nondipole as nd
+    p = nd.set_ground_state(nd.make_nondipole(kappa_max=6, l_max=2, n_r=30))
+    prop = Tdde(p)
+    assert prop.apply_path == "staged" and p.n_terms == 24
+    ops, fact = orc.assemble(p), orc.factor_precond(p)
+    x = rand_vec(p.n, 12)
+    xd = prop.to_device(x)
+    for alpha, beta, g in [(1.0, 0.5j * p.dt, p.g_mid(70)), (0.2 + 0.1j, 1.0 - 0.5j, np.linspace(-1.0, 1.0, p.n_terms))]:
+        y = prop.apply(alpha, beta, g, xd).cpu().numpy()
+        assert rel(y, orc.apply(ops, alpha, beta, np.asarray(g, float), x)) <= 1e-12
+    z = prop.precond(xd).cpu().numpy()
+    assert rel(z, orc.apply_precond(fact, x)) <= 1e-12
+    n_steps, first = 4, 60
+    c_ref, infos = orc.propagate(p, ops, fact, p.c0, n_steps, first_step=first)
+    c = prop.to_device(p.c0)
+    st = prop.propagate(c, p.g_table(n_steps, first_step=first))
+    assert st["steps"] == n_steps and st["status"] == 0
+    assert rel(c.cpu().numpy(), c_ref) <= 1e-9
+    assert abs(st["half_iters"] - sum(i.half_iters for i in infos)) <= n_steps
+    assert abs(prop.norm(c) - orc.s_norm_sq(ops, p.c0)) <= 1e-9
+    prop.close()
+
+
+def test_nondipole_kappa15_sampled_rows():
+    """kappa_max = 15 (480 channels, 24 terms, up to 11 couplings per row and term): outputs sampled against the oracle's
+    direct summation of the definition; S-norm conservation over a few steps under the field."""
+    from paper_2512_21697_b200 import Tdde
+    from tdde_inputs import nondipole as nd
+    p = nd.set_ground_state(nd.make_nondipole(kappa_max=15, l_max=2, n_r=40))
+    prop = Tdde(p)
+    assert prop.apply_path == "staged" and p.n_ang == 480
+    x = rand_vec(p.n, 13)
+    g = np.linspace(0.3, 1.1, p.n_terms)
+    y = prop.apply(1.0, 0.5j * p.dt, g, prop.to_device(x)).cpu().numpy().reshape(p.n_ang, p.n_rad)
+    rng = np.random.default_rng(2)
+    chan = np.concatenate([rng.integers(0, p.n_ang, 150), [0, 1, p.n_ang - 1, 127, 128, 255, 256]])
+    rad = np.concatenate([rng.integers(0, p.n_rad, 150), [0, p.n_rad - 1, 5, 13, 14, 40, 41]])
+    ref = orc.apply_rows_sampled(p, 1.0, 0.5j * p.dt, g, x, chan, rad)
+    assert np.max(np.abs(y[chan, rad] - ref)) <= 1e-12 * np.sqrt(np.mean(np.abs(ref) ** 2))
+    c = prop.to_device(p.c0)
+    n0 = prop.norm(c)
+    st = prop.propagate(c, p.g_table(3, first_step=60))
+    assert st["steps"] == 3 and st["status"] == 0 and st["half_iters"] >= 6
+    assert abs(prop.norm(c) - n0) <= 1e-9
+    prop.close()

@@ -497,3 +497,137 @@ def test_hydrogen_norm_conserved_under_field():
     assert abs(orc.s_norm_sq(ops, c) - n0) < 10 * p.n_steps * p.rtol * 10
     leaked = 1.0 - abs(np.vdot(c0, ops.S @ c)) ** 2
     assert leaked > 1e-6                              # the field really couples channels
+
+
+# ----------------------------------------------------------------------------- NEXT-1: paper-shaped angular operators (Eq. 17-18, 27-30)
+def test_clebsch_gordan_and_3j_vs_sympy_and_orthogonality():
+    """Racah-formula Clebsch-Gordan coefficients and 3j symbols of tdde_inputs.nondipole against sympy's exact values, and the
+    orthogonality sums every such table obeys."""
+    from sympy import N, Rational as Rq
+    from sympy.physics.wigner import clebsch_gordan as scg, wigner_3j as s3j
+    from tdde_inputs import nondipole as nd
+    for tj1, tj2 in [(2, 1), (6, 1), (3, 2), (5, 4), (20, 1), (31, 1)]:
+        for tJ in range(abs(tj1 - tj2), tj1 + tj2 + 1, 2):
+            for tm1 in range(-tj1, tj1 + 1, 2):
+                for tm2 in range(-tj2, tj2 + 1, 2):
+                    ref = float(N(scg(Rq(tj1, 2), Rq(tj2, 2), Rq(tJ, 2), Rq(tm1, 2), Rq(tm2, 2), Rq(tm1 + tm2, 2)), 30))
+                    assert abs(nd.clebsch_gordan(tj1, tm1, tj2, tm2, tJ, tm1 + tm2) - ref) < 1e-13
+    for l1, l2, l3 in [(2, 1, 1), (4, 2, 2), (7, 3, 4), (10, 10, 0), (12, 2, 14)]:
+        tot = 0.0
+        for m1 in range(-l1, l1 + 1):
+            for m2 in range(-l2, l2 + 1):
+                v = nd.wigner_3j(l1, l2, l3, m1, m2, -m1 - m2)
+                if abs(m1 + m2) <= l3:
+                    assert abs(v - float(N(s3j(l1, l2, l3, m1, m2, -m1 - m2), 30))) < 1e-13
+                tot += v * v
+        assert abs(tot - 1.0) < 1e-13                      # sum over m1, m2, m3 of (3j)^2 = 1
+    # unitarity of the coupling: sum_{m1} <j1 m1 j2 M-m1 | J M> <j1 m1 j2 M-m1 | J' M> = delta_{J J'}
+    tj1, tj2, tM = 8, 3, 3
+    Js = list(range(abs(tj1 - tj2), tj1 + tj2 + 1, 2))
+    G = np.array([[sum(nd.clebsch_gordan(tj1, tm1, tj2, tM - tm1, a, tM) * nd.clebsch_gordan(tj1, tm1, tj2, tM - tm1, b, tM)
+                       for tm1 in range(-tj1, tj1 + 1, 2)) for b in Js] for a in Js])
+    assert np.max(np.abs(G - np.eye(len(Js)))) < 1e-13
+
+
+def test_h_theta_by_quadrature_on_the_sphere():
+    """(H^theta_l)_{k'k mu'mu} = 4 pi Y_l0(z) <X_{-k',mu'}| sigma_x Y_l0 |X_{k,mu}> (Eq. 18) by brute force: spinor
+    components from sympy's Clebsch-Gordan coefficients and scipy's spherical harmonics, integrated with Gauss-Legendre x
+    uniform quadrature over the sphere -- no 3j symbol, no code of the generator."""
+    from scipy.special import sph_harm_y
+    from sympy import N, Rational as Rq
+    from sympy.physics.wigner import clebsch_gordan as scg
+    from tdde_inputs import nondipole as nd
+    from tdde_inputs.hydrogen import l_of_kappa
+    xg, wg = np.polynomial.legendre.leggauss(24)
+    phi = 2 * np.pi * np.arange(48) / 48
+    TH, PH = np.meshgrid(np.arccos(xg), phi, indexing="ij")
+    Wt = np.outer(wg, np.full(48, 2 * np.pi / 48))
+
+    def spinor(kappa, mu):                                  # (up, down) components on the grid
+        l, j = l_of_kappa(kappa), abs(kappa) - 0.5
+        comps = []
+        for ms in (0.5, -0.5):
+            m = mu - ms
+            if abs(m) > l:
+                comps.append(np.zeros_like(TH, dtype=complex))
+                continue
+            cg = float(N(scg(l, Rq(1, 2), Rq(int(2 * j), 2), int(round(m)), Rq(int(2 * ms), 2), Rq(int(round(2 * mu)), 2)), 20))
+            comps.append(cg * sph_harm_y(l, int(round(m)), TH, PH))
+        return comps
+
+    rng = np.random.default_rng(0)
+    cases = [(0, 1, 1, 0.5, -0.5), (0, -1, -1, -0.5, 0.5), (1, -1, -2, 0.5, 1.5), (1, 2, 1, -0.5, 0.5), (2, -2, 3, 1.5, 2.5), (2, 3, -3, -1.5, -0.5),
+             (3, -4, 2, 2.5, 1.5), (1, 1, 1, 0.5, -0.5), (2, -1, -1, 0.5, -0.5)]
+    for l, kp, k, mup, mu in cases:
+        bu, bd = spinor(-kp, mup)
+        ku, kd = spinor(k, mu)
+        yl0 = sph_harm_y(l, 0, TH, PH)
+        val = np.sum(Wt * yl0 * (np.conj(bu) * kd + np.conj(bd) * ku))          # sigma_x swaps the components
+        ref = 4 * np.pi * np.sqrt((2 * l + 1) / (4 * np.pi)) * val
+        got = nd.h_theta_element(l, kp, k, int(round(2 * mup)), int(round(2 * mu)))
+        assert abs(ref.imag) < 1e-12 and abs(got - ref.real) < 1e-12, (l, kp, k, mup, mu, got, ref)
+
+
+def test_h_theta_selection_rules_sum_rule_and_growth():
+    """Zero pattern = {mu = mu' +- 1} and the l-triangle / parity rule (Eq. 29-30); sigma_x^2 = 1 gives the sum
+    rule sum_{k mu} (H^theta_0)^2 = 1 per row whose partners all lie inside kappa_max; the number of non-zeros of the coupling
+    pattern grows like kappa_max^2 at fixed l_max (Fig. 2)."""
+    from tdde_inputs import nondipole as nd
+    from tdde_inputs.hydrogen import channel_list, l_of_kappa
+    _, chans, _ = channel_list(5)
+    for l in range(0, 4):
+        H = nd.h_theta(l, chans)
+        for i, (kp, mup) in enumerate(chans):
+            for j, (k, mu) in enumerate(chans):
+                allowed = abs(mu - mup) == 1.0 and nd.triangle_allows(l, kp, k)
+                full = nd.h_theta_element(l, kp, k, int(round(2 * mup)), int(round(2 * mu)))       # without the mu shortcut
+                assert abs(full - H[i, j]) < 1e-15
+                if not allowed:
+                    assert H[i, j] == 0.0 or abs(H[i, j]) < 1e-14, (l, kp, k, mup, mu)
+        assert np.count_nonzero(np.abs(H) > 1e-12) > 0
+    H0 = nd.h_theta(0, chans)
+    inner = [i for i, (kp, _) in enumerate(chans) if abs(kp) <= 3]          # sigma_x X_{k,mu} only reaches |kappa| + 1
+    assert np.max(np.abs(np.sum(H0[inner] ** 2, axis=1) - 1.0)) < 1e-13
+    # growth: the pattern is exactly the selection rules (just verified entry by entry), so count those for larger kappa_max
+    def rule_count(kmax, lmax):
+        kaps = [s * m for m in range(1, kmax + 1) for s in (-1, 1)]
+        tot = 0
+        for kp in kaps:
+            for k in kaps:
+                if not any(nd.triangle_allows(l, kp, k) for l in range(lmax + 1)):
+                    continue
+                # the spherical harmonics of both spinor components must exist: |m| <= l on each side, m = mu' + ms = mu - ms
+                lb, lk, jp, j = l_of_kappa(-kp), l_of_kappa(k), abs(kp) - 0.5, abs(k) - 0.5
+                for mup in np.arange(-jp, jp + 1):
+                    for ms in (-0.5, 0.5):
+                        tot += abs(mup + 2 * ms) <= j and abs(mup + ms) <= min(lb, lk)
+        return tot
+    _, ch, _ = channel_list(4)
+    pat = np.zeros((len(ch), len(ch)), dtype=bool)
+    for l in range(3):
+        pat |= np.abs(nd.h_theta(l, ch)) > 1e-13
+    assert int(pat.sum()) == rule_count(4, 2)
+    counts = [rule_count(kmax, 2) for kmax in (8, 16, 32, 64)]
+    ratios = [counts[i + 1] / counts[i] for i in range(3)]
+    assert all(3.7 < r < 4.7 for r in ratios) and abs(ratios[2] - 4.0) < 0.15, (counts, ratios)
+
+
+def test_nondipole_operator_hermitian_and_norm_conserving():
+    """Eq. 17: each bracket alone is not Hermitian, their sum is; the oracle's CN step then conserves the
+    S-norm under the field.  The panel-streamed apply agrees with the CSR apply on this non-banded, 24-term operator."""
+    from tdde_inputs import nondipole as nd
+    p = nd.make_nondipole(kappa_max=2, l_max=2, n_r=9)
+    g = p.g_mid(40)
+    assert np.all(g != 0.0) and p.n_terms == 24
+    HI = sum(gl * np.kron(csr_to_dense(t, p.n_ang), band_to_dense(t.R_band)) for gl, t in zip(g, p.terms))
+    assert np.linalg.norm(HI - HI.conj().T) <= 1e-13 * np.linalg.norm(HI)
+    first = sum(gl * np.kron(csr_to_dense(t, p.n_ang), band_to_dense(t.R_band)) for gl, t in zip(g[0::2], p.terms[0::2]))
+    assert np.linalg.norm(first - first.conj().T) > 1e-3 * np.linalg.norm(first)
+    p = nd.set_ground_state(nd.make_nondipole(kappa_max=3, l_max=2, n_r=12))
+    ops, fact = orc.assemble(p), orc.factor_precond(p)
+    c, infos = orc.propagate(p, ops, fact, p.c0, 4, first_step=60)
+    assert all(i.status == "ok" for i in infos) and max(i.half_iters for i in infos) >= 2
+    assert abs(orc.s_norm_sq(ops, c) - orc.s_norm_sq(ops, p.c0)) <= 40 * p.rtol
+    x = np.random.default_rng(3).standard_normal(2 * p.n).view(np.complex128)
+    gg = p.g_mid(60)
+    assert rel(orc.apply_panels(p, 1.0, 0.5j * p.dt, gg, x, panel=7), orc.apply(ops, 1.0, 0.5j * p.dt, gg, x)) < 1e-13
