@@ -20,6 +20,8 @@
  *   - every call returns 0 on success or a negative tdde_status; nothing throws or aborts across the ABI.
  *   - all device work is enqueued on the CUDA stream given to tdde_create.
  *   - there is no CPU fallback: every call fails with TDDE_ECUDA when no CUDA device is usable.
+ *   - a handle belongs to the device that was current at tdde_create; every call runs there whatever the caller's current device.
+ * Measurement helpers, test exports and the paper-variant comparator are declared in tdde_bench.h (compiled in with -DTDDE_WITH_BENCH).
  */
 #ifndef TDDE_H_
 #define TDDE_H_
@@ -114,37 +116,16 @@ int tdde_precond(tdde_handle* h, const tdde_c64* x_dev, tdde_c64* y_dev);
  * device, propagated and copied back; synchronises.  This is the end-to-end entry bench.py's "e2e" times. */
 int tdde_propagate_host(tdde_handle* h, tdde_c64* c_host, int64_t n_steps, const double* g_table, tdde_stats* st);
 
-/* Pin P11 support: one CN step that runs exactly n_iters full BiCGSTAB iterations with every exit test
- * disabled.  trace_dev (device, nullable): [n_iters][8][n] complex128 receiving, after each iteration, the
- * vectors p, v, s, t, x, r, y, z (this order, boundary layout).  Synchronises. */
-int tdde_step_forced(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, int32_t n_iters, tdde_c64* trace_dev);
-
-/* Measurement helpers (timed in bench.py; no effect on state).
- *   tdde_time_kernel: enqueue `reps` launches of one internal kernel on the handle's stream between two CUDA
- *   events and return the mean milliseconds per launch in *ms_out.  which: 0 = operator apply v = A y with
- *   fused <rhat,v>; 1 = preconditioner apply; 2 = p-update; 3 = s-update; 4 = x,r-update; 5 = boundary<->internal
- *   transpose; 6 = S-only apply (norm).  g: host [n_terms] used by which == 0.  Synchronises.
- *   tdde_fp64_peak: run an unrolled independent-DFMA kernel on every SM and return achieved FLOP/s. */
-int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, const double* g, double* ms_out);
-int tdde_fp64_peak(void* cuda_stream, double* flops_out);
-
-/* Comparator, not on the product path: the paper's own formulation on this GPU.  Allocates the global
- * CSR matrix A = S + i dt/2 H(g) (structure once), recomputes every non-zero from the stored radial and
- * angular matrices with one assembly kernel and forms y = A x by CSR SpMV, `reps` times
- * each; mean milliseconds go to *ms_assemble / *ms_spmv (host, nullable), the non-zero count to *nnz (host, nullable).
- * x_dev, y_dev: device, n complex128, boundary layout, must not alias.  Needs 20 bytes of device memory per non-zero.
- * Only for problems on the banded apply path (tdde_apply_path == 1), else TDDE_EINVAL.  Synchronises. */
-int tdde_paper_variant(tdde_handle* h, const double* g, const tdde_c64* x_dev, tdde_c64* y_dev, int32_t reps,
-                       double* ms_assemble, double* ms_spmv, int64_t* nnz);
-
-/* Host-only self-test of the set-up code behind tdde_precond (no GPU needed): builds a random banded
- * M = S + i tau H of size n and half-bandwidth w, the partitioned factors for P partitions, replays the
- * solve on the host and writes the relative residual ||M y - b|| / ||b|| to *rel_res (host).  Returns the number of
- * partitions actually used (>= 1; the plan shrinks P until interiors are >= 8 w rows) or a negative tdde_status. */
-int tdde_selftest_partition(int32_t n, int32_t w, int32_t P, uint32_t seed, double* rel_res);
-
-/* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
-int64_t tdde_launch_count(const tdde_handle* h);
+/* Observables (Eq. 33: dP/dE = sum_{kappa,mu} |<psi_{kappa,mu,E}|Psi>|^2 with psi the field-free
+ * eigenstates of PAPER.md:174-184, Eq. 19-20, which depend on kappa only).
+ * tdde_set_eigenstates copies n_states eigenvectors per kappa-class to the device: V host [n_cls][n_states][n_rad], row e of class k =
+ *   eigenvector e of the pencil (H0_k, S_k), normalised as the caller wants the probabilities normalised (v^H S_k v = 1 for
+ *   probabilities).  The eigen-solve itself is set-up work on 2 kappa_max banded pencils of size n_rad and is left to the caller
+ *   (LAPACK); this library evaluates the projections, which touch the whole state.
+ * tdde_project: P_host [n_ang][n_states] receives |v_{k(a),e}^H S_k c_a|^2 for every channel a (the inner product of the
+ *   non-orthogonal basis).  c_dev: device, n complex128.  Synchronises.  TDDE_EINVAL before tdde_set_eigenstates. */
+int tdde_set_eigenstates(tdde_handle* h, int32_t n_states, const tdde_c64* V);
+int tdde_project(tdde_handle* h, const tdde_c64* c_dev, double* P_host);
 
 /* Which operator-apply kernel the handle uses: 1 = banded A_L held in registers, 2 = general sparse A_L staged in shared memory
  * (x tile by TMA), 0 = unstaged generic CSR fall-back. */
@@ -153,7 +134,7 @@ int tdde_apply_path(const tdde_handle* h);
 void        tdde_destroy(tdde_handle* h);          /* NULL is allowed */
 const char* tdde_strerror(int status);             /* static string */
 const char* tdde_last_cuda_error(void);            /* text of the last CUDA failure seen by this thread */
-int         tdde_version(void);                    /* ABI version, currently 1 */
+int         tdde_version(void);                    /* ABI version, currently 2 */
 
 #ifdef __cplusplus
 }

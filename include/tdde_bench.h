@@ -1,0 +1,48 @@
+/* tdde_bench.h -- measurement helpers, test exports and the same-box comparator of libtdde.so.  None of these is on the product
+ * path (tdde.h); they are compiled into the library only with -DTDDE_WITH_BENCH (paper_2512_21697_b200/build.py sets it; a
+ * production build can leave it out) and are what bench.py and tests/ call. */
+#ifndef TDDE_BENCH_H_
+#define TDDE_BENCH_H_
+
+#include "tdde.h"
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Pin P11 support: one CN step that runs exactly n_iters full BiCGSTAB iterations with every exit test
+ * disabled.  trace_dev (device, nullable): [n_iters][8][n] complex128 receiving, after each iteration, the
+ * vectors p, v, s, t, x, r, y, z (this order, boundary layout).  Synchronises. */
+int tdde_step_forced(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, int32_t n_iters, tdde_c64* trace_dev);
+
+/* Measurement helpers (timed in bench.py; no effect on state).
+ *   tdde_time_kernel: enqueue `reps` launches of one internal kernel on the handle's stream between two CUDA
+ *   events and return the mean milliseconds per launch in *ms_out.  which: 0 = operator apply v = A y with
+ *   fused <rhat,v>; 1 = preconditioner apply; 2 = p-update; 3 = s-update; 4 = x,r-update; 5 = boundary<->internal
+ *   transpose; 6 = S-only apply (norm).  g: host [n_terms] used by which == 0.  Synchronises.
+ *   tdde_fp64_peak: run an unrolled independent-DFMA kernel on every SM and return achieved FLOP/s. */
+int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, const double* g, double* ms_out);
+int tdde_fp64_peak(void* cuda_stream, double* flops_out);
+
+/* Comparator, not on the product path: the paper's own formulation on this GPU.  Allocates the global
+ * CSR matrix A = S + i dt/2 H(g) (structure once), recomputes every non-zero from the stored radial and
+ * angular matrices with one assembly kernel and forms y = A x by CSR SpMV, `reps` times
+ * each; mean milliseconds go to *ms_assemble / *ms_spmv (host, nullable), the non-zero count to *nnz (host, nullable).
+ * x_dev, y_dev: device, n complex128, boundary layout, must not alias.  Needs 20 bytes of device memory per non-zero.
+ * Only for problems on the banded apply path (tdde_apply_path == 1), else TDDE_EINVAL.  Synchronises. */
+int tdde_paper_variant(tdde_handle* h, const double* g, const tdde_c64* x_dev, tdde_c64* y_dev, int32_t reps,
+                       double* ms_assemble, double* ms_spmv, int64_t* nnz);
+
+/* Host-only self-test of the set-up code behind tdde_precond (no GPU needed): builds a random banded
+ * M = S + i tau H of size n and half-bandwidth w, the partitioned factors for P partitions, replays the
+ * solve on the host and writes the relative residual ||M y - b|| / ||b|| to *rel_res (host).  Returns the number of
+ * partitions actually used (>= 1; the plan shrinks P until interiors are >= 8 w rows) or a negative tdde_status. */
+int tdde_selftest_partition(int32_t n, int32_t w, int32_t P, uint32_t seed, double* rel_res);
+
+/* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
+int64_t tdde_launch_count(const tdde_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TDDE_BENCH_H_ */

@@ -126,6 +126,21 @@ def s_norm_sq(ops: Operators, c: np.ndarray) -> float:
     return float(np.real(np.vdot(c, ops.S @ c)))
 
 
+def project(problem, V: np.ndarray, c: np.ndarray) -> np.ndarray:
+    """P[a, e] = |<psi_{k(a), e} | Psi_a>|^2 = |v_e^H S_k c_a|^2, the terms of dP/dE (Eq. 33) before the sum over
+    (kappa, mu); V[k, e, :] are eigenvectors of the field-free pencil (H0_k, S_k) (Eq. 19-20)."""
+    from_band = lambda band: sum(np.diag(band[max(0, -d):band.shape[0] - max(0, d), d + (band.shape[1] - 1) // 2], d)
+                                 for d in range(-(band.shape[1] - 1) // 2, (band.shape[1] - 1) // 2 + 1))
+    C = c.reshape(problem.n_ang, problem.n_rad)
+    out = np.zeros((problem.n_ang, V.shape[1]))
+    for k in range(problem.n_cls):
+        Sk = from_band(problem.S_band[k])
+        idx = np.nonzero(problem.cls_of_chan == k)[0]
+        amp = (V[k].conj() @ (Sk @ C[idx].T))            # [n_states, channels of the class]
+        out[idx] = (np.abs(amp) ** 2).T
+    return out
+
+
 # ----------------------------------------------------------------------------- sampled rows (P10)
 def apply_rows_sampled(problem, alpha: complex, beta: complex, g: np.ndarray, x: np.ndarray,
                        chan: np.ndarray, rad: np.ndarray) -> np.ndarray:

@@ -19,7 +19,7 @@ LIB_PATH = os.environ.get("TDDE_LIB_PATH", os.path.join(_HERE, "libtdde.so"))
 EXPORTS = [
     "tdde_create", "tdde_step", "tdde_propagate", "tdde_norm", "tdde_apply", "tdde_precond",
     "tdde_propagate_host", "tdde_step_forced", "tdde_time_kernel", "tdde_fp64_peak", "tdde_launch_count",
-    "tdde_apply_path", "tdde_selftest_partition", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
+    "tdde_apply_path", "tdde_set_eigenstates", "tdde_project", "tdde_selftest_partition", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
 ]
 
 STATUS = {0: "TDDE_OK", -1: "TDDE_EINVAL", -2: "TDDE_ENOMEM", -3: "TDDE_ECUDA", -4: "TDDE_ESINGULAR",
@@ -81,6 +81,10 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.tdde_launch_count.argtypes = [vp]
     lib.tdde_launch_count.restype = i64
     lib.tdde_apply_path.argtypes = [vp]
+    lib.tdde_set_eigenstates.argtypes = [vp, i32, vp]
+    lib.tdde_set_eigenstates.restype = C.c_int
+    lib.tdde_project.argtypes = [vp, vp, vp]
+    lib.tdde_project.restype = C.c_int
     lib.tdde_selftest_partition.argtypes = [i32, i32, i32, C.c_uint32, C.POINTER(dbl)]
     lib.tdde_selftest_partition.restype = C.c_int
     lib.tdde_paper_variant.argtypes = [vp, vp, vp, vp, i32, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i64)]
@@ -218,6 +222,20 @@ class Tdde:
                                        C.c_void_p(tr.data_ptr()) if trace else None)
         _check(self.lib, rc, "tdde_step_forced")
         return tr
+
+    def set_eigenstates(self, V: np.ndarray):
+        """V[k, e, :] = eigenvector e of the pencil (H0_k, S_k) of kappa-class k (tdde_set_eigenstates)."""
+        V = np.ascontiguousarray(V, dtype=np.complex128)
+        if V.ndim != 3 or V.shape[2] != self.n_rad:
+            raise ValueError("V must have shape [n_cls, n_states, n_rad]")
+        self._n_states = V.shape[1]
+        _check(self.lib, self.lib.tdde_set_eigenstates(self.h, V.shape[1], _np_ptr(V)), "tdde_set_eigenstates")
+
+    def project(self, c_dev) -> np.ndarray:
+        """P[a, e] = |v_{k(a),e}^H S c_a|^2 (tdde_project; Eq. 33 before the sum over channels)."""
+        out = np.empty((self.n_ang, self._n_states), dtype=np.float64)
+        _check(self.lib, self.lib.tdde_project(self.h, self._vec(c_dev), _np_ptr(out)), "tdde_project")
+        return out
 
     def time_kernel(self, which: int, reps: int, g=None) -> float:
         garr = _g_array(g, self.n_terms) if (g is not None and self.n_terms) else np.zeros(max(1, self.n_terms))

@@ -166,11 +166,16 @@ __global__ void __launch_bounds__(SP_NC, 1) k_apply_sparse(const __grid_constant
           cplx z0 = make_double2(0, 0), z1 = make_double2(0, 0);
           const int ns = p.sp_nslot[L];
           int q = 0;
-          for (; q + 1 < ns; q += 2, s += 2) {
-            cfma(z0, Av[(size_t)s * astr], xw0[Ac[(size_t)s * astr]]);
-            cfma(z1, Av[(size_t)(s + 1) * astr], xw0[Ac[(size_t)(s + 1) * astr]]);
+          constexpr int U = W >= 13 ? 4 : 8;                  // loads in flight per thread (the rows of A_L may come from L2)
+          for (; q + U <= ns; q += U, s += U) {
+            cplx av[U];
+            int ci[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) { av[u] = Av[(size_t)(s + u) * astr]; ci[u] = Ac[(size_t)(s + u) * astr]; }
+#pragma unroll
+            for (int u = 0; u < U; u += 2) { cfma(z0, av[u], xw0[ci[u]]); cfma(z1, av[u + 1], xw0[ci[u + 1]]); }
           }
-          if (q < ns) { cfma(z0, Av[(size_t)s * astr], xw0[Ac[(size_t)s * astr]]); ++s; }
+          for (; q < ns; ++q, ++s) cfma(z0, Av[(size_t)s * astr], xw0[Ac[(size_t)s * astr]]);
           const cplx z = cmul(coefL[L], cadd(z0, z1));
           const cplx* rc = st + ((size_t)r * T + L) * ND;    // warp-uniform: broadcast LDS.128
 #pragma unroll

@@ -108,7 +108,7 @@ extern "C" void tdde_destroy(tdde_handle* h) {
   if (!h) return;
   DeviceGuard dg(h->device);
   cudaStreamSynchronize(h->stream);
-  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_pslot, h->d_warp_cls, h->d_spval, h->d_spcol, h->d_Wsp, h->d_Corner, h->d_Schur, h->d_rsm, h->d_rsp, h->d_Lcol, h->d_Ucol, h->X, h->r,
+  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_eig, h->d_proj, h->d_pslot, h->d_warp_cls, h->d_spval, h->d_spcol, h->d_Wsp, h->d_Corner, h->d_Schur, h->d_rsm, h->d_rsp, h->d_Lcol, h->d_Ucol, h->X, h->r,
                   h->rhat, h->p, h->v, h->s, h->t, h->y, h->z, h->c_stage, h->d_st, h->d_st_bench, h->d_partials,
                   h->d_ticket, h->d_g, h->d_g_small, h->d_zero_g};
   for (void* p : ptrs) if (p) cudaFree(p);

@@ -274,6 +274,7 @@ extern "C" int tdde_propagate_host(tdde_handle* h, tdde_c64* c_host, int64_t n_s
   return rc;
 }
 
+#ifdef TDDE_WITH_BENCH
 extern "C" int tdde_step_forced(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, int32_t n_iters, tdde_c64* trace_dev) {
   if (!h || !c_dev || n_iters < 0 || (h->cfg.n_terms > 0 && !g_mid)) return TDDE_EINVAL;
   DeviceGuard dg(h->device);
@@ -304,6 +305,8 @@ extern "C" int tdde_step_forced(tdde_handle* h, tdde_c64* c_dev, const double* g
   CU(cudaStreamSynchronize(h->stream));
   return status;
 }
+
+#endif  // TDDE_WITH_BENCH
 
 extern "C" int tdde_norm(tdde_handle* h, const tdde_c64* c_dev, double* out) {
   if (!h || !c_dev || !out) return TDDE_EINVAL;

@@ -56,6 +56,11 @@ struct tdde_handle {
   bool have_xmaps = false;
   cplx* c_stage = nullptr;                   // boundary-layout device buffer for tdde_propagate_host
 
+  // observables (tdde_project): eigenvectors [n_cls][n_rad][n_states] and the probability buffer [n_ang][n_states]
+  cplx* d_eig = nullptr;
+  double* d_proj = nullptr;
+  int n_states = 0;
+
   // solver state, scratch
   SolverState* d_st = nullptr;
   SolverState* d_st_bench = nullptr;         // never-idle dummy state for tdde_time_kernel

@@ -10,6 +10,9 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include "tdde.h"
+#ifdef TDDE_WITH_BENCH
+#include "tdde_bench.h"
+#endif
 
 #define TDDE_MAX_TERMS 24
 #define TDDE_MAX_PARTIAL_BLOCKS 65536

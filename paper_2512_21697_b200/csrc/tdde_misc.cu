@@ -1,6 +1,8 @@
 // tdde_misc.cu -- measurement helpers and small exports of tdde.h.
 #include <cstring>
+#include <vector>
 #include "tdde_handle.h"
+#include "tdde_reduce.cuh"
 
 extern "C" const char* tdde_strerror(int status) {
   switch (status) {
@@ -16,9 +18,11 @@ extern "C" const char* tdde_strerror(int status) {
 }
 
 extern "C" const char* tdde_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
-extern "C" int tdde_version(void) { return 1; }
-extern "C" int64_t tdde_launch_count(const tdde_handle* h) { return h ? h->launches : 0; }
+extern "C" int tdde_version(void) { return 2; }
 extern "C" int tdde_apply_path(const tdde_handle* h) { return h ? h->path : -1; }
+
+#ifdef TDDE_WITH_BENCH
+extern "C" int64_t tdde_launch_count(const tdde_handle* h) { return h ? h->launches : 0; }
 
 extern "C" int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, const double* g, double* ms_out) {
   if (!h || !ms_out || reps <= 0 || which < 0 || which > 6) return TDDE_EINVAL;
@@ -85,6 +89,69 @@ extern "C" int tdde_fp64_peak(void* cuda_stream, double* flops_out) {
   cudaFree(d);
   const double fmas = (double)blocks * threads * (double)iters * 64.0;   // 8 chains x 8 unrolled
   *flops_out = 2.0 * fmas / (ms * 1e-3);
+  CU(cudaGetLastError());
+  return 0;
+}
+
+#endif  // TDDE_WITH_BENCH
+
+// ---- observables (Eq. 33) ----
+// P[a][e] = |sum_j conj(V_k(a)[j][e]) u[j][a]|^2 with u = S c in the internal layout.  Thread = channel (coalesced reads of u),
+// PJ_NE states per thread; the eigenvector entries of a row are contiguous in e and (per kappa-class) warp-uniform.
+#define PJ_NE 8
+__global__ void __launch_bounds__(128) k_project(const cplx* __restrict__ u, const cplx* __restrict__ V, const int* __restrict__ cls,
+                                                  double* __restrict__ P, int n_ang, int n_rad, int ld, int n_states) {
+  const int a = blockIdx.x * 128 + threadIdx.x;
+  if (a >= n_ang) return;
+  const int e0 = blockIdx.y * PJ_NE;
+  const cplx* Vk = V + (size_t)cls[a] * n_rad * n_states + e0;
+  const int ne = min(PJ_NE, n_states - e0);
+  cplx acc[PJ_NE];
+#pragma unroll
+  for (int e = 0; e < PJ_NE; ++e) acc[e] = make_double2(0, 0);
+  for (int j = 0; j < n_rad; ++j) {
+    const cplx uj = u[(size_t)j * ld + a];
+    const cplx* vr = Vk + (size_t)j * n_states;
+#pragma unroll
+    for (int e = 0; e < PJ_NE; ++e)
+      if (e < ne) cfma_conj(acc[e], __ldg(vr + e), uj);
+  }
+  for (int e = 0; e < ne; ++e) P[(size_t)a * n_states + e0 + e] = acc[e].x * acc[e].x + acc[e].y * acc[e].y;
+}
+
+extern "C" int tdde_set_eigenstates(tdde_handle* h, int32_t n_states, const tdde_c64* V) {
+  if (!h || n_states <= 0 || !V) return TDDE_EINVAL;
+  DeviceGuard dg(h->device);
+  const int n_cls = h->cfg.n_cls, n_rad = h->cfg.n_rad;
+  CU(cudaStreamSynchronize(h->stream));
+  if (h->d_eig) { cudaFree(h->d_eig); h->d_eig = nullptr; }
+  if (h->d_proj) { cudaFree(h->d_proj); h->d_proj = nullptr; }
+  h->n_states = 0;
+  // [k][e][j] at the boundary -> [k][j][e] on the device (the kernel walks j and wants the states of a row contiguous)
+  std::vector<zc> T((size_t)n_cls * n_rad * n_states);
+  const zc* Vh = reinterpret_cast<const zc*>(V);
+  for (int k = 0; k < n_cls; ++k)
+    for (int e = 0; e < n_states; ++e)
+      for (int j = 0; j < n_rad; ++j) T[((size_t)k * n_rad + j) * n_states + e] = Vh[((size_t)k * n_states + e) * n_rad + j];
+  CU(cudaMalloc((void**)&h->d_eig, T.size() * sizeof(cplx)));
+  CU(cudaMemcpy(h->d_eig, T.data(), T.size() * sizeof(cplx), cudaMemcpyHostToDevice));
+  CU(cudaMalloc((void**)&h->d_proj, (size_t)h->cfg.n_ang * n_states * sizeof(double)));
+  h->n_states = n_states;
+  return 0;
+}
+
+extern "C" int tdde_project(tdde_handle* h, const tdde_c64* c_dev, double* P_host) {
+  if (!h || !c_dev || !P_host || h->n_states <= 0) return TDDE_EINVAL;
+  DeviceGuard dg(h->device);
+  int rc;
+  h->launches += launch_to_internal(reinterpret_cast<const cplx*>(c_dev), h->y, h->cfg.n_ang, h->cfg.n_rad, h->ld, h->stream);
+  // u = S c: the S-only operator apply (beta = 0), no fused reduction
+  if ((rc = enqueue_apply(h, h->y, h->z, nullptr, BLK_S, make_double2(0, 0), false, h->d_zero_g, nullptr, 0, FIN_NONE, h->d_st))) return rc;
+  dim3 grid((h->cfg.n_ang + 127) / 128, (h->n_states + PJ_NE - 1) / PJ_NE);
+  k_project<<<grid, 128, 0, h->stream>>>(h->z, h->d_eig, h->d_cls, h->d_proj, h->cfg.n_ang, h->cfg.n_rad, h->ld, h->n_states);
+  h->launches += 1;
+  CU(cudaMemcpyAsync(P_host, h->d_proj, (size_t)h->cfg.n_ang * h->n_states * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
   CU(cudaGetLastError());
   return 0;
 }

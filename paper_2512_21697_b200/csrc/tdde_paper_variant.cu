@@ -1,3 +1,4 @@
+#ifdef TDDE_WITH_BENCH
 // tdde_paper_variant.cu -- the paper's own formulation on the same GPU, as a comparator:
 //   * the global matrix A(t) = S + i dt/2 H(t) is held in CSR, structure allocated once;
 //   * an assembly kernel recomputes every non-zero from the stored radial matrices and angular couplings each step,
@@ -158,3 +159,5 @@ extern "C" int tdde_paper_variant(tdde_handle* h, const double* g, const tdde_c6
   cleanup();
   return 0;
 }
+
+#endif  // TDDE_WITH_BENCH

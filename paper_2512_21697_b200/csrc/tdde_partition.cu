@@ -193,6 +193,7 @@ bool build_partitioned_factors(const std::vector<zc>& Mrow, const PartitionPlan&
   return true;
 }
 
+#ifdef TDDE_WITH_BENCH
 // ---- host self-test (no GPU): the partitioned solve, with the device kernels P1/P2/P3 replayed in plain loops on the
 // host arrays exactly as laid out for the device; checked by the residual of the original banded system ----
 extern "C" int tdde_selftest_partition(int32_t n, int32_t w, int32_t P, uint32_t seed, double* max_rel_err) {
@@ -302,3 +303,4 @@ extern "C" int tdde_selftest_partition(int32_t n, int32_t w, int32_t P, uint32_t
   *max_rel_err = std::sqrt(num / den);
   return pl.P;        // the partition count actually used (>= 1)
 }
+#endif  // TDDE_WITH_BENCH

@@ -695,3 +695,32 @@ def test_nondipole_kappa15_sampled_rows():
     assert st["steps"] == 3 and st["status"] == 0 and st["half_iters"] >= 6
     assert abs(prop.norm(c) - n0) <= 1e-9
     prop.close()
+
+
+def test_projection_on_eigenstates_next4(hyd):
+    """tdde_project (Eq. 33): |<psi_{kappa,e}| S |c_a>|^2 for every channel and eigenstate, against the
+    oracle; on the hydrogen basis the propagated 1s state keeps its weight on the 1s eigenstate when the field is off."""
+    import scipy.linalg as sla
+    p, prop, ops, fact = hyd
+    V = np.zeros((p.n_cls, p.n_rad, p.n_rad), dtype=np.complex128)
+    for k, kap in enumerate(p.meta["kappas"]):
+        S, H = p.meta["dense"][kap]
+        _, vec = sla.eigh(H, S)
+        V[k] = vec.T
+    prop.set_eigenstates(V)
+    x = rand_vec(p.n, 17)
+    P = prop.project(prop.to_device(x))
+    ref = orc.project(p, V, x)
+    assert np.max(np.abs(P - ref)) <= 1e-12 * np.max(ref)
+    c = prop.to_device(p.c0)
+    prop.propagate(c, np.zeros((10, p.n_terms)))
+    P = prop.project(c)
+    a = p.meta["chans"].index((-1, 0.5))
+    S1, H1 = p.meta["dense"][-1]
+    E1 = sla.eigh(H1, S1, eigvals_only=True)
+    j = int(np.nonzero(E1 > -p.meta["c"] ** 2)[0][0])
+    assert abs(P[a, j] - 1.0) <= 1e-9 and abs(P.sum() - 1.0) <= 1e-9
+    # fewer states than basis functions
+    prop.set_eigenstates(V[:, 5:45, :])
+    P2 = prop.project(prop.to_device(x))
+    assert np.max(np.abs(P2 - ref[:, 5:45])) <= 1e-12 * np.max(ref)

@@ -631,3 +631,36 @@ def test_nondipole_operator_hermitian_and_norm_conserving():
     x = np.random.default_rng(3).standard_normal(2 * p.n).view(np.complex128)
     gg = p.g_mid(60)
     assert rel(orc.apply_panels(p, 1.0, 0.5j * p.dt, gg, x, panel=7), orc.apply(ops, 1.0, 0.5j * p.dt, gg, x)) < 1e-13
+
+
+# ----------------------------------------------------------------------------- NEXT-4: projection on field-free eigenstates (Eq. 33)
+def _eigenbasis(p):
+    """Eigenvectors of every kappa-class pencil (H0_k, S_k) by LAPACK (scipy.linalg.eigh), S-orthonormal: V[k, e, :]."""
+    V = np.zeros((p.n_cls, p.n_rad, p.n_rad), dtype=np.complex128)
+    E = np.zeros((p.n_cls, p.n_rad))
+    for k in range(p.n_cls):
+        E[k], vec = sla.eigh(band_to_dense(p.H0_band[k]), band_to_dense(p.S_band[k]))
+        V[k] = vec.T
+    return E, V
+
+
+def test_projection_on_eigenstates_delta_and_completeness():
+    """oracle.project: an eigenstate projects onto itself only (S-orthonormality of the generalised eigenvectors), and over the
+    full eigenbasis of a channel the probabilities add up to that channel's share of the S-norm (completeness)."""
+    p = make_synthetic(n_ang=9, n_r=12, bandwidth=7, n_terms=0, dt=0.01, n_steps=1, rtol=1e-10, seed=2)
+    E, V = _eigenbasis(p)
+    c = np.zeros(p.n, dtype=np.complex128)
+    a0, e0 = 5, 7
+    c[a0 * p.n_rad:(a0 + 1) * p.n_rad] = (0.6 + 0.8j) * V[p.cls_of_chan[a0], e0]
+    P = orc.project(p, V, c)
+    ref = np.zeros_like(P)
+    ref[a0, e0] = 1.0
+    assert np.max(np.abs(P - ref)) < 1e-12
+    rng = np.random.default_rng(1)
+    x = rng.standard_normal(2 * p.n).view(np.complex128)
+    P = orc.project(p, V, x)
+    ops = orc.assemble(p)
+    X = x.reshape(p.n_ang, p.n_rad)
+    per_chan = np.array([np.real(np.vdot(X[a], band_to_dense(p.S_band[p.cls_of_chan[a]]) @ X[a])) for a in range(p.n_ang)])
+    assert np.max(np.abs(P.sum(axis=1) - per_chan)) < 1e-11 * per_chan.max()
+    assert abs(P.sum() - orc.s_norm_sq(ops, x)) < 1e-11 * P.sum()
