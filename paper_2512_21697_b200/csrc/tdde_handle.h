@@ -108,6 +108,7 @@ enum BlkSel { BLK_S = 0, BLK_H0 = 1, BLK_MP = 2, BLK_TMP = 3 };
 int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int blk, cplx beta, bool with_terms,
                   const double* g_dev, const int* step_ptr, int guard, int fin, SolverState* st,
                   const cplx* addv = nullptr, int emode = 0, cplx oscale = cplx{1.0, 0.0}, cplx* y2 = nullptr);
-int enqueue_precond(tdde_handle* h, const cplx* x, cplx* y, const SolverState* st);
+int enqueue_precond(tdde_handle* h, const cplx* x, cplx* y, const SolverState* st, bool spikes_done = false);
+int enqueue_vec_update(tdde_handle* h, int mode, SolverState* st, bool* fused);   // mode 0: p-update, 1: s-update (+ spike products when fused)
 VecArgs make_vec_args(tdde_handle* h, SolverState* st, int fin);
 int sync_state(tdde_handle* h);

@@ -162,6 +162,7 @@ struct PrecArgs {
   const int* aslot;        // [ld] the apply's per-CTA class slot (128-channel groups), used by k_precond_spikes
   const int* cta_cls;      // [n_cta][TDDE_AP_MAXC]
   const SolverState* st;   // nullable guard
+  int spikes_done;         // 1: rsm / rsp already hold the spike products of x (formed by k_vec_spikes): skip P1
 };
 
 __host__ __device__ inline int pc_lo(const PrecArgs& p, int q) { return q * (p.int_base + p.w) + (q < p.int_rem ? q : p.int_rem); }
@@ -175,7 +176,8 @@ int launch_apply_generic(const ApplyArgs& a, int num_sms, cudaStream_t s);
 int launch_apply_sparse(const ApplyArgs& a, int W, cudaStream_t s);
 size_t apply_sparse_smem(int W, int T, int nslots, int xw, bool a_in_smem);
 int launch_precond(const PrecArgs& a, cudaStream_t s);
-size_t precond_tile_smem(int w, int tile_rows);   // dynamic shared memory of k_precond_tile
+size_t precond_tile_smem(int w, int tile_rows);
+int launch_vec_spikes(const VecArgs& v, const PrecArgs& a, int mode, cudaStream_t s);   // dynamic shared memory of k_precond_tile
 int launch_vec_p(const VecArgs& a, cudaStream_t s);
 int launch_vec_s(const VecArgs& a, cudaStream_t s);
 int launch_vec_halfexit(const VecArgs& a, cudaStream_t s);

@@ -41,12 +41,18 @@ extern "C" int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, con
   CU(cudaEventCreate(&e1));
   const cplx itau = make_double2(0.0, h->tau);
   int rc = 0;
+  bool fused_avail = false, fused_tmp = false;
+  if (which == 1) {                                 // does the fused update exist for this problem?  (also fills rsm / rsp)
+    if ((rc = enqueue_vec_update(h, 0, sb, &fused_avail))) return rc;
+  }
   auto once = [&]() -> int {
     switch (which) {
       case 0: return enqueue_apply(h, h->y, h->v, h->rhat, BLK_MP, itau, true, h->d_g_small, nullptr, 0, FIN_ALPHA, sb, h->p);   // as the iteration runs it
-      case 1: return enqueue_precond(h, h->p, h->y, nullptr);
-      case 2: h->launches += launch_vec_p(make_vec_args(h, sb, FIN_NONE), s); return 0;
-      case 3: h->launches += launch_vec_s(make_vec_args(h, sb, FIN_NONE), s); return 0;
+      // 1-3 as an iteration runs them: the p- and s-updates carry the spike products of the solve that follows (when available),
+      // and the solve then starts at its Schur step
+      case 1: return enqueue_precond(h, h->p, h->y, nullptr, fused_avail);
+      case 2: return enqueue_vec_update(h, 0, sb, &fused_tmp);
+      case 3: return enqueue_vec_update(h, 1, sb, &fused_tmp);
       case 4: h->launches += launch_vec_xr(make_vec_args(h, sb, FIN_NONE), s); return 0;
       case 5: h->launches += launch_to_internal(h->z, h->t, h->cfg.n_ang, h->cfg.n_rad, h->ld, s); return 0;
       default: return enqueue_apply(h, h->y, h->z, h->y, BLK_S, make_double2(0, 0), false, h->d_zero_g, nullptr, 0, FIN_NONE, sb);

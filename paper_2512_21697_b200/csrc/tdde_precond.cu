@@ -114,6 +114,123 @@ __global__ void __launch_bounds__(128) k_precond_spikes(const PrecArgs p) {
   }
 }
 
+// ---- P1 fused into the BiCGSTAB vector updates that PRODUCE the right-hand side of the solve: the p-update
+// (MODE 0: p = r + beta (p - omega v), first iteration p = r) or the s-update (MODE 1: s = r - alpha v with ||s||^2) runs on a
+// (128 channels x interior) decomposition and forms the spike dot products of the vector it has just computed, so the solve
+// never re-reads its right-hand side for them.  CTA (bx, q) also updates the separator rows after interior q. ----
+#define VSP_ROWS 4
+template <int W, int MODE>
+__global__ void __launch_bounds__(128) k_vec_spikes(const VecArgs v, const PrecArgs p) {
+  const SolverState* st = v.red.st;
+  if (solver_idle(st)) return;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cplx* Ws = reinterpret_cast<cplx*>(smem_raw);                      // [2][TDDE_AP_MAXC][VSP_ROWS][2W]
+  constexpr int CH = VSP_ROWS * 2 * W;
+  const int tid = threadIdx.x, ld = p.ld;
+  const int a = blockIdx.x * 128 + tid;
+  const bool ok = a < ld;
+  const int ac = ok ? a : ld - 1;
+  const int q = blockIdx.y;
+  const int lo = pc_lo(p, q), len = pc_len(p, q);
+  const int nrows = len + (q + 1 < p.P ? W : 0);                     // interior + the separator after it
+  const int* ccls = p.cta_cls + blockIdx.x * TDDE_AP_MAXC;
+  int ncls = 0;
+#pragma unroll
+  for (int c = 0; c < TDDE_AP_MAXC; ++c) ncls += (ccls[c] >= 0);
+  const int slot = p.aslot[ac];
+  const cplx* Wg = p.Wsp + ((size_t)p.cls[ac] * p.n_rad + lo) * 2 * W;
+  const int nch = (nrows + VSP_ROWS - 1) / VSP_ROWS;
+  auto issue = [&](int c) {
+    const int r0 = c * VSP_ROWS, nr = min(VSP_ROWS, len - r0);       // spike rows exist for interior rows only
+    if (nr > 0) {
+      cplx* dst0 = Ws + (size_t)(c & 1) * TDDE_AP_MAXC * CH;
+      for (int s = 0; s < ncls; ++s) {
+        const cplx* src = p.Wsp + ((size_t)ccls[s] * p.n_rad + lo + r0) * 2 * W;
+        for (int e = tid; e < nr * 2 * W; e += 128) cp_async16(dst0 + s * CH + e, src + e);
+      }
+    }
+    cp_async_commit();
+  };
+  const bool first = st->first;
+  const cplx beta = st->beta, omega = st->omega, alpha = st->alpha;
+  const size_t base = (size_t)lo * ld + ac;
+  const cplx *rin = v.r + base, *vin = v.v + base;
+  cplx* pio = (MODE == 0 ? v.p : v.s) + base;
+  cplx rn[VSP_ROWS], vn[VSP_ROWS], pn[VSP_ROWS];
+  auto fetch = [&](int c) {
+    const int r0 = c * VSP_ROWS;
+#pragma unroll
+    for (int r = 0; r < VSP_ROWS; ++r) {
+      const bool in = r0 + r < nrows;
+      rn[r] = in ? rin[(size_t)(r0 + r) * ld] : make_double2(0, 0);
+      if (MODE == 1 || !first) vn[r] = in ? vin[(size_t)(r0 + r) * ld] : make_double2(0, 0);
+      if (MODE == 0 && !first) pn[r] = in ? pio[(size_t)(r0 + r) * ld] : make_double2(0, 0);
+    }
+  };
+  issue(0);
+  fetch(0);
+  cplx am[W], ap[W];
+#pragma unroll
+  for (int c = 0; c < W; ++c) am[c] = ap[c] = make_double2(0, 0);
+  double s2 = 0;
+  for (int c = 0; c < nch; ++c) {
+    const int r0 = c * VSP_ROWS, nr = min(VSP_ROWS, nrows - r0), nri = min(VSP_ROWS, len - r0);
+    cplx b[VSP_ROWS];
+#pragma unroll
+    for (int r = 0; r < VSP_ROWS; ++r) {
+      if (MODE == 0) {
+        b[r] = rn[r];
+        if (!first) {
+          cplx t = pn[r];
+          cfms(t, omega, vn[r]);                                     // p - omega v
+          cfma(b[r], beta, t);
+        }
+      } else {
+        b[r] = rn[r];
+        cfms(b[r], alpha, vn[r]);
+        if (r < nr && ok) { s2 = fma(b[r].x, b[r].x, s2); s2 = fma(b[r].y, b[r].y, s2); }
+      }
+    }
+    issue(c + 1);
+    if (c + 1 < nch) fetch(c + 1);
+    if (ok) {
+#pragma unroll
+      for (int r = 0; r < VSP_ROWS; ++r)
+        if (r < nr) pio[(size_t)(r0 + r) * ld] = b[r];
+    }
+    cp_async_wait<1>();
+    __syncthreads();
+    if (nri > 0) {
+      const cplx* wl = Ws + (size_t)(c & 1) * TDDE_AP_MAXC * CH + (size_t)(slot >= 0 ? slot : 0) * CH;
+      if (slot >= 0) {
+#pragma unroll
+        for (int r = 0; r < VSP_ROWS; ++r) {
+          if (r < nri) {
+#pragma unroll
+            for (int e = 0; e < W; ++e) { cfma(am[e], wl[r * 2 * W + e], b[r]); cfma(ap[e], wl[r * 2 * W + W + e], b[r]); }
+          }
+        }
+      } else {
+        for (int r = 0; r < nri; ++r) {
+          const cplx* wr = Wg + (size_t)(r0 + r) * 2 * W;
+#pragma unroll
+          for (int e = 0; e < W; ++e) { cfma(am[e], __ldg(wr + e), b[r]); cfma(ap[e], __ldg(wr + W + e), b[r]); }
+        }
+      }
+    }
+    __syncthreads();
+  }
+  cp_async_wait<0>();
+  if (ok) {
+#pragma unroll
+    for (int c = 0; c < W; ++c) {
+      p.rsm[((size_t)q * W + c) * ld + a] = am[c];
+      p.rsp[((size_t)q * W + c) * ld + a] = ap[c];
+    }
+  }
+  if (MODE == 1) grid_reduce_finalize<128>(0.0, 0.0, s2, v.red);
+}
+
 // ---- P2: block Thomas over the separators.  CTA = 32 channels x W warps; warp c owns row c of every w x w block product,
 // lane = channel.  r_j = b_S(j) - r(+)_j - r(-)_{j+1};
 //   forward   r'_j = r_j - (B_j D'^-1_{j-1}) r'_{j-1},  z_j = D'^-1_j r'_j   (z_j kept in the r(+) scratch)
@@ -461,15 +578,44 @@ static int launch_precond_w(const PrecArgs& a, cudaStream_t s) {
   if (cudaFuncSetAttribute(k_precond_tile<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -2;
   int n = 0;
   if (a.P > 1) {
-    const size_t ssmem = (size_t)2 * TDDE_AP_MAXC * SPK_ROWS * 2 * W * sizeof(cplx);
-    if (cudaFuncSetAttribute(k_precond_spikes<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ssmem) != cudaSuccess) return -2;
-    k_precond_spikes<W><<<dim3((a.ld + 127) / 128, a.P), 128, ssmem, s>>>(a);
+    if (!a.spikes_done) {
+      const size_t ssmem = (size_t)2 * TDDE_AP_MAXC * SPK_ROWS * 2 * W * sizeof(cplx);
+      if (cudaFuncSetAttribute(k_precond_spikes<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ssmem) != cudaSuccess) return -2;
+      k_precond_spikes<W><<<dim3((a.ld + 127) / 128, a.P), 128, ssmem, s>>>(a);
+      ++n;
+    }
     k_precond_schur<W><<<a.ld / PC_NT, PC_NT * W, 0, s>>>(a);
     k_precond_corners<W><<<dim3((a.ld + 127) / 128, (a.P - 1) * W), 128, 0, s>>>(a);
-    n = 3;
+    n += 2;
   }
   k_precond_tile<W><<<dim3(a.ld / PC_NT, a.P), PC_NT, smem, s>>>(a);
   return n + 1;
+}
+
+template <int W>
+static int launch_vec_spikes_w(const VecArgs& v, const PrecArgs& a, int mode, cudaStream_t s) {
+  const size_t smem = (size_t)2 * TDDE_AP_MAXC * VSP_ROWS * 2 * W * sizeof(cplx);
+  dim3 grid((a.ld + 127) / 128, a.P);
+  if (mode == 0) {
+    if (cudaFuncSetAttribute(k_vec_spikes<W, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -2;
+    k_vec_spikes<W, 0><<<grid, 128, smem, s>>>(v, a);
+  } else {
+    if (cudaFuncSetAttribute(k_vec_spikes<W, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -2;
+    k_vec_spikes<W, 1><<<grid, 128, smem, s>>>(v, a);
+  }
+  return 1;
+}
+
+// the p-update (mode 0) or the s-update (mode 1) fused with the spike products of the vector it writes; -1: not available
+// for this problem (no partitions, or an untemplated bandwidth): the caller runs the plain update and the full solve
+int launch_vec_spikes(const VecArgs& v, const PrecArgs& a, int mode, cudaStream_t s) {
+  if (a.P <= 1 || (long long)((a.ld + 127) / 128) * a.P > TDDE_MAX_PARTIAL_BLOCKS) return -1;
+  switch (a.w) {
+#define X(W) case W: return launch_vec_spikes_w<W>(v, a, mode, s);
+    TDDE_PC_WIDTHS(X)
+#undef X
+    default: return -1;
+  }
 }
 
 size_t precond_tile_smem(int w, int tile_rows) {
