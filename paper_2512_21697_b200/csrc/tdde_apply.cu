@@ -128,7 +128,7 @@ __device__ __forceinline__ void apply_group(const ApplyArgs& p, const ApplyCommo
   using PL = ApplyPlan<T, M0, MS, W, NG, BLK>;
   constexpr int ND = PL::ND, MAXM = PL::MAXM, NS = SH::nslots(), XW = PL::XW, JC = PL::JC, GM = PL::gmaxm(G);
   constexpr bool SPLIT = (NG == 2) && (T > 0);
-  constexpr int RU = TDDE_AP_RU;                             // rows unrolled together (register pressure vs ILP)
+  constexpr int RU = (W >= 9 && T > 0) ? 1 : ((T == 0) ? 4 : TDDE_AP_RU);   // rows unrolled together (register pressure vs ILP)
   const int ld = k.ld;
 
   // angular coefficients of this group's terms in registers, pre-multiplied by beta * g_L

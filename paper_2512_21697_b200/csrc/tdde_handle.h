@@ -94,6 +94,14 @@ struct DeviceGuard {
   ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
 };
 
+// a CUDA event that is destroyed on every exit path
+struct ScopedEvent {
+  cudaEvent_t e = nullptr;
+  cudaError_t create() { return cudaEventCreate(&e); }
+  ~ScopedEvent() { if (e) cudaEventDestroy(e); }
+  operator cudaEvent_t() const { return e; }
+};
+
 extern thread_local std::string g_last_cuda_error;
 int tdde_cuda_fail(cudaError_t e, const char* what);
 

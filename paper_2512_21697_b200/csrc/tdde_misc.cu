@@ -36,9 +36,9 @@ extern "C" int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, con
   for (cplx* v : vecs) h->launches += launch_fill(v, h->nint, seed++, s);
   if (h->cfg.n_terms > 0 && g)
     CU(cudaMemcpyAsync(h->d_g_small, g, h->cfg.n_terms * sizeof(double), cudaMemcpyHostToDevice, s));
-  cudaEvent_t e0, e1;
-  CU(cudaEventCreate(&e0));
-  CU(cudaEventCreate(&e1));
+  ScopedEvent e0, e1;
+  CU(e0.create());
+  CU(e1.create());
   const cplx itau = make_double2(0.0, h->tau);
   int rc = 0;
   bool fused_avail = false, fused_tmp = false;
@@ -68,8 +68,6 @@ extern "C" int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, con
     CU(cudaEventElapsedTime(&ms, e0, e1));
     *ms_out = (double)ms / reps;
   }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
   CU(cudaGetLastError());
   return rc;
 }
@@ -81,17 +79,15 @@ extern "C" int tdde_fp64_peak(void* cuda_stream, double* flops_out) {
   CU(cudaMalloc((void**)&d, sizeof(double)));
   const int blocks = tdde_num_sms() * 8, threads = 256, iters = 4096;
   launch_dfma_peak(d, blocks, threads, 64, s);
-  cudaEvent_t e0, e1;
-  CU(cudaEventCreate(&e0));
-  CU(cudaEventCreate(&e1));
+  ScopedEvent e0, e1;
+  CU(e0.create());
+  CU(e1.create());
   CU(cudaEventRecord(e0, s));
   launch_dfma_peak(d, blocks, threads, iters, s);
   CU(cudaEventRecord(e1, s));
   CU(cudaEventSynchronize(e1));
   float ms = 0;
   CU(cudaEventElapsedTime(&ms, e0, e1));
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
   cudaFree(d);
   const double fmas = (double)blocks * threads * (double)iters * 64.0;   // 8 chains x 8 unrolled
   *flops_out = 2.0 * fmas / (ms * 1e-3);

@@ -137,8 +137,8 @@ extern "C" int tdde_paper_variant(tdde_handle* h, const double* g, const tdde_c6
   k_pv_rowptr<<<blocks, 256, 0, s>>>(p, n, nnz);
   k_pv_assemble<0><<<blocks, 256, 0, s>>>(p, n);                      // structure: once
   h->launches += 2;
-  cudaEvent_t e0, e1, e2;
-  PV(cudaEventCreate(&e0)); PV(cudaEventCreate(&e1)); PV(cudaEventCreate(&e2));
+  ScopedEvent e0, e1, e2;
+  PV(e0.create()); PV(e1.create()); PV(e2.create());
   k_pv_assemble<1><<<blocks, 256, 0, s>>>(p, n);                      // warm-up
   k_pv_spmv<<<blocks, 256, 0, s>>>(p, n, reinterpret_cast<const cplx*>(x_dev), reinterpret_cast<cplx*>(y_dev));
   PV(cudaEventRecord(e0, s));
@@ -153,7 +153,6 @@ extern "C" int tdde_paper_variant(tdde_handle* h, const double* g, const tdde_c6
   PV(cudaEventElapsedTime(&ts, e1, e2));
   if (ms_assemble) *ms_assemble = ta / reps;
   if (ms_spmv) *ms_spmv = ts / reps;
-  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(e2);
   PV(cudaGetLastError());
 #undef PV
   cleanup();
