@@ -120,12 +120,19 @@ int tdde_propagate_host(tdde_handle* h, tdde_c64* c_host, int64_t n_steps, const
  * eigenstates of PAPER.md:174-184, Eq. 19-20, which depend on kappa only).
  * tdde_set_eigenstates copies n_states eigenvectors per kappa-class to the device: V host [n_cls][n_states][n_rad], row e of class k =
  *   eigenvector e of the pencil (H0_k, S_k), normalised as the caller wants the probabilities normalised (v^H S_k v = 1 for
- *   probabilities).  The eigen-solve itself is set-up work on 2 kappa_max banded pencils of size n_rad and is left to the caller
- *   (LAPACK); this library evaluates the projections, which touch the whole state.
+ *   probabilities), e.g. the output of tdde_eigensolve.
+ * tdde_eigensolve (no handle needed): ALL eigenpairs of the n_cls Hermitian-definite pencils (H0_k, S_k) of PAPER.md Eq. 20 on the current
+ *   device, batched over the classes (banded Cholesky of S_k, reduction to standard form, cyclic Jacobi with the round-robin parallel
+ *   ordering, back-transformation).  S_band, H0_band: host [n_cls][n_rad][2*w0+1] as for tdde_create; E_host [n_cls][n_rad] ascending;
+ *   V_host (nullable) [n_cls][n_rad][n_rad], row e = eigenvector of E[e], S-orthonormal -- the layout tdde_set_eigenstates takes.
+ *   Set-up work (the paper solves these once, "2 kappa_max separate eigenvalue problems of dimension 2N"): dense O(n_rad^3) per class,
+ *   n_rad <= 4096.  TDDE_ESINGULAR when some S_k is not positive definite.  Synchronises.
  * tdde_project: P_host [n_ang][n_states] receives |v_{k(a),e}^H S_k c_a|^2 for every channel a (the inner product of the
  *   non-orthogonal basis).  c_dev: device, n complex128.  Synchronises.  TDDE_EINVAL before tdde_set_eigenstates. */
 int tdde_set_eigenstates(tdde_handle* h, int32_t n_states, const tdde_c64* V);
 int tdde_project(tdde_handle* h, const tdde_c64* c_dev, double* P_host);
+int tdde_eigensolve(int32_t n_cls, int32_t n_rad, int32_t w0, const tdde_c64* S_band, const tdde_c64* H0_band, double* E_host,
+                    tdde_c64* V_host, void* cuda_stream);
 
 /* Which operator-apply kernel the handle uses: 1 = banded A_L held in registers, 2 = general sparse A_L staged in shared memory
  * (x tile by TMA), 0 = unstaged generic CSR fall-back. */

@@ -126,6 +126,21 @@ def s_norm_sq(ops: Operators, c: np.ndarray) -> float:
     return float(np.real(np.vdot(c, ops.S @ c)))
 
 
+def eigenstates(problem):
+    """Field-free eigenstates per kappa-class: H0_k psi = E S_k psi (Eq. 19-20 with reading R3), by LAPACK's
+    generalised Hermitian-definite solver on the dense blocks.  Returns E [n_cls, n_rad] ascending and V [n_cls, n_rad, n_rad] with
+    V[k, e, :] the S-orthonormal eigenvector of E[k, e]."""
+    import scipy.linalg as sla
+    dense = lambda band: sum(np.diag(band[max(0, -d):band.shape[0] - max(0, d), d + (band.shape[1] - 1) // 2], d)
+                             for d in range(-(band.shape[1] - 1) // 2, (band.shape[1] - 1) // 2 + 1))
+    E = np.zeros((problem.n_cls, problem.n_rad))
+    V = np.zeros((problem.n_cls, problem.n_rad, problem.n_rad), dtype=np.complex128)
+    for k in range(problem.n_cls):
+        E[k], vec = sla.eigh(dense(problem.H0_band[k]), dense(problem.S_band[k]))
+        V[k] = vec.T
+    return E, V
+
+
 def project(problem, V: np.ndarray, c: np.ndarray) -> np.ndarray:
     """P[a, e] = |<psi_{k(a), e} | Psi_a>|^2 = |v_e^H S_k c_a|^2, the terms of dP/dE (Eq. 33) before the sum over
     (kappa, mu); V[k, e, :] are eigenvectors of the field-free pencil (H0_k, S_k) (Eq. 19-20)."""

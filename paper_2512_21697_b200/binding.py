@@ -19,7 +19,7 @@ LIB_PATH = os.environ.get("TDDE_LIB_PATH", os.path.join(_HERE, "libtdde.so"))
 EXPORTS = [
     "tdde_create", "tdde_step", "tdde_propagate", "tdde_norm", "tdde_apply", "tdde_precond",
     "tdde_propagate_host", "tdde_step_forced", "tdde_time_kernel", "tdde_fp64_peak", "tdde_launch_count",
-    "tdde_apply_path", "tdde_set_eigenstates", "tdde_project", "tdde_selftest_partition", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
+    "tdde_apply_path", "tdde_set_eigenstates", "tdde_project", "tdde_eigensolve", "tdde_selftest_partition", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
 ]
 
 STATUS = {0: "TDDE_OK", -1: "TDDE_EINVAL", -2: "TDDE_ENOMEM", -3: "TDDE_ECUDA", -4: "TDDE_ESINGULAR",
@@ -85,6 +85,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.tdde_set_eigenstates.restype = C.c_int
     lib.tdde_project.argtypes = [vp, vp, vp]
     lib.tdde_project.restype = C.c_int
+    lib.tdde_eigensolve.argtypes = [i32, i32, i32, vp, vp, vp, vp, vp]
+    lib.tdde_eigensolve.restype = C.c_int
     lib.tdde_selftest_partition.argtypes = [i32, i32, i32, C.c_uint32, C.POINTER(dbl)]
     lib.tdde_selftest_partition.restype = C.c_int
     lib.tdde_paper_variant.argtypes = [vp, vp, vp, vp, i32, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i64)]
@@ -119,6 +121,25 @@ def _g_array(g, n_terms: int, rows: Optional[int] = None) -> np.ndarray:
     if g.size != want:
         raise ValueError(f"g has {g.size} entries, expected {want}")
     return g
+
+
+def eigensolve(S_band: np.ndarray, H0_band: np.ndarray, want_vectors: bool = True, stream=None):
+    """All eigenpairs of the per-class pencils (H0_k, S_k) on the GPU (tdde_eigensolve): returns (E [n_cls, n_rad] ascending,
+    V [n_cls, n_rad, n_rad] with V[k, e, :] the S-orthonormal eigenvector of E[k, e], or None)."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("no CUDA device: the TDDE library has no CPU fallback")
+    lib = load_library()
+    S = np.ascontiguousarray(S_band, dtype=np.complex128)
+    H = np.ascontiguousarray(H0_band, dtype=np.complex128)
+    n_cls, n_rad, nd = S.shape
+    E = np.empty((n_cls, n_rad), dtype=np.float64)
+    V = np.empty((n_cls, n_rad, n_rad), dtype=np.complex128) if want_vectors else None
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = lib.tdde_eigensolve(n_cls, n_rad, (nd - 1) // 2, _np_ptr(S), _np_ptr(H), _np_ptr(E), _np_ptr(V) if want_vectors else None,
+                             C.c_void_p(st.cuda_stream))
+    _check(lib, rc, "tdde_eigensolve")
+    return E, V
 
 
 class Tdde:

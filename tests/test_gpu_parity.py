@@ -724,3 +724,47 @@ def test_projection_on_eigenstates_next4(hyd):
     prop.set_eigenstates(V[:, 5:45, :])
     P2 = prop.project(prop.to_device(x))
     assert np.max(np.abs(P2 - ref[:, 5:45])) <= 1e-12 * np.max(ref)
+
+
+def test_device_eigensolve_next4(hyd):
+    """tdde_eigensolve (Eq. 19-20): all eigenpairs of the eight hydrogen pencils (H0_k, S_k), n_rad = 400,
+    against LAPACK through the oracle, the Sommerfeld closed form for the bound levels, the pencil residual and S-orthonormality;
+    the device's own eigenvectors then feed tdde_project."""
+    from paper_2512_21697_b200 import eigensolve
+    p, prop, ops, fact = hyd
+    E_ref, V_ref = orc.eigenstates(p)
+    E, V = eigensolve(p.S_band, p.H0_band)
+    scale = np.max(np.abs(E_ref))                              # ~ 2 c^2 + the stiffest pseudo-continuum state
+    assert np.max(np.abs(E - E_ref)) <= 1e-12 * scale
+    c2 = p.meta["c"] ** 2
+    k1 = p.meta["kappas"].index(-1)
+    e1s = E[k1][E[k1] > -c2][0]
+    assert abs(e1s - c2 * (np.sqrt(1.0 - 1.0 / c2) - 1.0)) <= 1e-9          # Dirac 1s1/2: c^2 (sqrt(1 - (Z/c)^2) - 1)
+    for k in range(p.n_cls):
+        S, H = tdde_inputs.band_to_dense(p.S_band[k]), tdde_inputs.band_to_dense(p.H0_band[k])
+        R = H @ V[k].T - (S @ V[k].T) * E[k][None, :]
+        assert np.linalg.norm(R) <= 1e-11 * np.linalg.norm(H) * np.sqrt(p.n_rad)
+        assert np.max(np.abs(V[k].conj() @ S @ V[k].T - np.eye(p.n_rad))) <= 1e-9
+    # projections with the device's eigenvectors: the same probabilities as with LAPACK's up to the conditioning of individual
+    # eigenvectors (eps |H| / gap: the spectrum spans 2 c^2 with gaps far below 1), and the same total per channel to rounding
+    prop.set_eigenstates(V)
+    x = rand_vec(p.n, 23)
+    P = prop.project(prop.to_device(x))
+    P_ref = orc.project(p, V_ref, x)
+    assert np.max(np.abs(P - P_ref)) <= 1e-6 * np.max(P)
+    assert np.max(np.abs(P.sum(axis=1) - P_ref.sum(axis=1))) <= 1e-10 * np.max(P_ref.sum(axis=1))
+    # a complex Hermitian pencil with a ragged size (odd n: one bye per Jacobi round)
+    q = tdde_inputs.make_synthetic(name="eig", n_ang=5, n_r=23, bandwidth=7, n_terms=0, dt=0.01, n_steps=1, rtol=1e-10, seed=9, with_c0=False)
+    q.S_band = q.S_band[:, :45].copy(); q.H0_band = q.H0_band[:, :45].copy()
+    for band in (q.S_band, q.H0_band):                        # entries pointing outside the truncated matrix are ignored by contract
+        w = q.w0
+        for i in range(45):
+            for d in range(-w, w + 1):
+                if i + d < 0 or i + d >= 45:
+                    band[:, i, d + w] = 0.0
+    q.n_rad = 45
+    Eq_ref, _ = orc.eigenstates(q)
+    Eq, Vq = eigensolve(q.S_band, q.H0_band)
+    assert np.max(np.abs(Eq - Eq_ref)) <= 1e-12 * np.max(np.abs(Eq_ref))
+    S, H = tdde_inputs.band_to_dense(q.S_band[2]), tdde_inputs.band_to_dense(q.H0_band[2])
+    assert np.linalg.norm(H @ Vq[2].T - (S @ Vq[2].T) * Eq[2][None, :]) <= 1e-12 * np.linalg.norm(H) * 45

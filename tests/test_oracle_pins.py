@@ -664,3 +664,22 @@ def test_projection_on_eigenstates_delta_and_completeness():
     per_chan = np.array([np.real(np.vdot(X[a], band_to_dense(p.S_band[p.cls_of_chan[a]]) @ X[a])) for a in range(p.n_ang)])
     assert np.max(np.abs(P.sum(axis=1) - per_chan)) < 1e-11 * per_chan.max()
     assert abs(P.sum() - orc.s_norm_sq(ops, x)) < 1e-11 * P.sum()
+
+
+def test_oracle_eigenstates_match_closed_form_and_pencil(hyd):
+    """oracle.eigenstates on the hydrogen blocks: the bound levels are the Sommerfeld closed form (golden file, P5), every pair
+    satisfies H v = E S v, and the vectors are S-orthonormal."""
+    p = hyd
+    E, V = orc.eigenstates(p)
+    c2 = p.meta["c"] ** 2
+    levels = read_golden_levels()
+    k1 = p.meta["kappas"].index(-1)
+    pos = E[k1][E[k1] > -c2]
+    assert abs(pos[0] - levels["1s1/2"][2]) < 1e-9 and abs(pos[1] - levels["2s1/2"][2]) < 1e-9
+    k2 = p.meta["kappas"].index(-2)
+    assert abs(E[k2][E[k2] > -c2][0] - levels["2p3/2"][2]) < 1e-9
+    for k in (0, 3):
+        S, H = band_to_dense(p.S_band[k]), band_to_dense(p.H0_band[k])
+        R = H @ V[k].T - (S @ V[k].T) * E[k][None, :]
+        assert np.linalg.norm(R) <= 1e-9 * np.linalg.norm(H)
+        assert np.max(np.abs(V[k].conj() @ S @ V[k].T - np.eye(p.n_rad))) < 1e-9
