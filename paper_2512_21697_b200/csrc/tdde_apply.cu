@@ -77,9 +77,13 @@ struct ApplyPlan {
   // BLK == false (in-iteration applies): the fused-dot operand and the vector replacing the block part reach the row loop
   // through a per-thread cp.async double buffer instead of plain global loads inside it
   static constexpr bool VST = !BLK && T > 0;
+  // W >= 9: the 2W+1-entry window and all A_L registers do not fit 255 registers.  Each warp group keeps the row of its widest
+  // term in shared memory instead (one column per thread, conflict-free 16-byte loads) -- no spills.
+  static constexpr bool ASM = W >= 9 && T > 0;
+  static constexpr int AS = ASM ? NG * 2 * MAXM * AP_NC : 0;
   __host__ __device__ static constexpr size_t smem_for(int jc) {
     return (size_t)(3 * (jc * T * ND + (BLK ? AP_MAXC * jc * ND : 0) + jc * XW) + ((T > 0 && NG == 2) ? 2 * jc * AP_NC : 0) +
-                    (VST ? 4 * jc * AP_NC : 0)) * sizeof(cplx) + 64;
+                    (VST ? 4 * jc * AP_NC : 0) + AS) * sizeof(cplx) + 64;
   }
   static constexpr int JC = (NG == 2 && smem_for(2 * AP_JC) <= 220 * 1024) ? 2 * AP_JC : AP_JC;
   static constexpr int RS = JC * T * ND;                    // complex elements
@@ -89,7 +93,7 @@ struct ApplyPlan {
   static constexpr int PS = (T > 0 && NG == 2) ? 2 * JC * AP_NC : 0;
   static constexpr int VS = VST ? 4 * JC * AP_NC : 0;       // [2 buffers][aux, addv][JC][AP_NC]
   static constexpr int NSTAGE = 3;
-  static constexpr size_t SMEM = (size_t)(NSTAGE * STAGE + PS + VS) * sizeof(cplx) + 64;
+  static constexpr size_t SMEM = (size_t)(NSTAGE * STAGE + PS + VS + AS) * sizeof(cplx) + 64;
   // Term split: the terms of one channel are shared between two warp groups so that each thread keeps only about
   // half of the A_L registers (4 warps per SM sub-partition instead of 2).  Group 0 also owns the block part, the
   // write-out and the fused inner products.  Greedy balance of complex FMAs per row, largest term first.
@@ -102,6 +106,11 @@ struct ApplyPlan {
     return mk;
   }
   __host__ __device__ static constexpr bool mine(int G, int L) { return NG == 1 || ((mask() >> L) & 1) == G; }
+  __host__ __device__ static constexpr int wide(int G) {     // the group's widest term (its A_L row lives in shared memory when ASM)
+    int best = -1;
+    for (int L = 0; L < T; ++L) if (mine(G, L) && (best < 0 || SH::m(L) > SH::m(best))) best = L;
+    return best;
+  }
   __host__ __device__ static constexpr int gmaxm(int G) {    // largest channel offset the group touches
     int m = 0;
     for (int L = 0; L < T; ++L) if (mine(G, L) && SH::m(L) > m) m = SH::m(L);
@@ -115,6 +124,7 @@ struct ApplyCommon {
   cplx* stage_base;
   cplx* Ps;
   cplx* Vs;
+  cplx* As;             // ASM: [NG][2 MAXM][AP_NC] row of each group's widest term
   uint64_t* full;       // [NSTAGE] TMA landed
   uint64_t* pfull;      // [2] group 1 has published its partial rows of a chunk
   uint64_t* pempty;     // [2] group 0 has consumed them
@@ -128,11 +138,13 @@ __device__ __forceinline__ void apply_group(const ApplyArgs& p, const ApplyCommo
   using PL = ApplyPlan<T, M0, MS, W, NG, BLK>;
   constexpr int ND = PL::ND, MAXM = PL::MAXM, NS = SH::nslots(), XW = PL::XW, JC = PL::JC, GM = PL::gmaxm(G);
   constexpr bool SPLIT = (NG == 2) && (T > 0);
-  constexpr int RU = (W >= 9 && T > 0) ? 1 : ((T == 0) ? 4 : TDDE_AP_RU);   // rows unrolled together (register pressure vs ILP)
+  constexpr int RU = (W >= 9 && T > 0) ? TDDE_AP_RU9 : ((T == 0) ? 4 : TDDE_AP_RU);   // rows unrolled together (register pressure vs ILP)
   const int ld = k.ld;
 
   // angular coefficients of this group's terms in registers, pre-multiplied by beta * g_L
   cplx Areg[NS > 0 ? NS : 1];
+  constexpr int LW = PL::ASM ? PL::wide(G) : -1;
+  cplx* const As = k.As + (size_t)G * 2 * MAXM * AP_NC + k.tid;   // this thread's column
   if (T > 0) {
     const double* g = p.g + (p.step_ptr ? (size_t)(*p.step_ptr) * T : 0);
 #pragma unroll
@@ -143,7 +155,8 @@ __device__ __forceinline__ void apply_group(const ApplyArgs& p, const ApplyCommo
 #pragma unroll
       for (int q = 0; q < 2 * SH::m(L); ++q) {
         const int s = SH::slot0(L) + q;
-        Areg[s] = cmul(coef, p.Aoff[(size_t)s * ld + k.ac]);
+        if (L == LW) As[q * AP_NC] = cmul(coef, p.Aoff[(size_t)s * ld + k.ac]);
+        else Areg[s] = cmul(coef, p.Aoff[(size_t)s * ld + k.ac]);
       }
     }
   }
@@ -224,7 +237,8 @@ __device__ __forceinline__ void apply_group(const ApplyArgs& p, const ApplyCommo
               if (PL::mine(G, L) && SH::m(L) >= (o < 0 ? -o : o)) {
                 // slot order within a term: o = -m..-1 -> q = o + m ; o = 1..m -> q = m + o - 1
                 const int q = o < 0 ? o + SH::m(L) : SH::m(L) + o - 1;
-                cfma(z[L], Areg[SH::slot0(L) + q], xo);
+                if (L == LW) cfma(z[L], As[q * AP_NC], xo);
+                else cfma(z[L], Areg[SH::slot0(L) + q], xo);
               }
             }
           }
@@ -278,7 +292,8 @@ __global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB
   k.stage_base = reinterpret_cast<cplx*>(smem_raw);
   k.Ps = k.stage_base + (size_t)PL::NSTAGE * PL::STAGE;
   k.Vs = k.Ps + PL::PS;
-  k.full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)(PL::NSTAGE * PL::STAGE + PL::PS + PL::VS) * sizeof(cplx));
+  k.As = k.Vs + PL::VS;
+  k.full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)(PL::NSTAGE * PL::STAGE + PL::PS + PL::VS + PL::AS) * sizeof(cplx));
   k.pfull = k.full + PL::NSTAGE;
   k.pempty = k.pfull + 2;
 

@@ -32,6 +32,9 @@
 #ifndef TDDE_AP_RU
 #define TDDE_AP_RU 2
 #endif
+#ifndef TDDE_AP_RU9
+#define TDDE_AP_RU9 1    // rows unrolled together for W >= 9
+#endif
 #ifndef TDDE_AP_MAXC
 #define TDDE_AP_MAXC 16    // banded apply: distinct kappa-classes per CTA staged in shared memory
 #endif
