@@ -439,6 +439,15 @@ __global__ void __launch_bounds__(AP_NT) k_apply_generic(const ApplyArgs p) {
   X(5, 1, 1, 6) \
   X(7, 1, 1, 3) X(7, 1, 1, 6) X(7, 1, 1, 9)
 
+// the instantiated shapes (T, M0, MS, W), for the structure fit at create
+int apply_banded_shapes(int (*out)[4], int cap) {
+  int n = 0;
+#define X(t, a, b, w) if (n < cap) { out[n][0] = t; out[n][1] = a; out[n][2] = b; out[n][3] = w; ++n; }
+  TDDE_BANDED_SHAPES(X)
+#undef X
+  return n;
+}
+
 bool apply_banded_available(int T, int m0, int mstep, int W) {
 #define X(t, a, b, w) if (T == t && (t == 0 || (m0 == a && mstep == b)) && W == w) return true;
   TDDE_BANDED_SHAPES(X)

@@ -1,5 +1,6 @@
 // tdde_create.cu -- tdde_create / tdde_destroy: validation, band repacking, per-class banded LU (host, one-time),
 // device allocation.  SURVEY 8(a) a0; PAPER.md:211-215 (Eq. 26), :268, :275-276 ("performed at start-up").
+#include <algorithm>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -70,36 +71,52 @@ int validate(const tdde_config* c, const tdde_c64* S, const tdde_c64* H0, const 
   return 0;
 }
 
-// Is every A_L banded with offsets 1..m_L, m_L = m0 + ms * L, and is a kernel instantiated for that shape?
-bool detect_banded(const tdde_config* c, const tdde_term* terms, int* m0, int* ms) {
+// Structure fit for the register-resident banded kernel: every A_L non-zero only at channel offsets 1 <= |o| <= m_L (no diagonal,
+// no duplicates).  The kernels are instantiated for a few shapes (T, m_L = M0 + MS L, W); the problem fits a shape when it has no more
+// terms, each term's reach is covered by a distinct slot, and every band is no wider than W.  The cheapest fitting shape is taken;
+// unused slots, unused offsets and the extra diagonals are zero-filled (wasted FMAs, but no change of kernel).
+struct BandFit { int T, m0, ms, W, slot_of[TDDE_MAX_TERMS]; };
+
+bool fit_banded(const tdde_config* c, const tdde_term* terms, BandFit* f) {
   const int T = c->n_terms;
-  if (!apply_banded_available(0, 0, 0, c->w0)) return false;   // the S-only apply needs the T = 0 kernel too
-  if (T == 0) { *m0 = *ms = 0; return true; }
-  int m[TDDE_MAX_TERMS];
+  int reach[TDDE_MAX_TERMS], order[TDDE_MAX_TERMS], maxw = c->w0;
   for (int L = 0; L < T; ++L) {
-    if (terms[L].w != c->w0) return false;
-    m[L] = 0;
+    maxw = std::max(maxw, (int)terms[L].w);
+    reach[L] = 0;
     for (int a = 0; a < c->n_ang; ++a)
       for (int q = terms[L].A_rowptr[a]; q < terms[L].A_rowptr[a + 1]; ++q) {
         const int o = terms[L].A_col[q] - a;
         if (o == 0) return false;
-        m[L] = std::max(m[L], std::abs(o));
-      }
-    if (m[L] == 0) return false;
-  }
-  // duplicates in a CSR row would need summing: reject (generic path sums them naturally)
-  for (int L = 0; L < T; ++L)
-    for (int a = 0; a < c->n_ang; ++a)
-      for (int q = terms[L].A_rowptr[a] + 1; q < terms[L].A_rowptr[a + 1]; ++q)
-        for (int q2 = terms[L].A_rowptr[a]; q2 < q; ++q2)
+        reach[L] = std::max(reach[L], std::abs(o));
+        for (int q2 = terms[L].A_rowptr[a]; q2 < q; ++q2)       // duplicates would need summing (the staged path does)
           if (terms[L].A_col[q] == terms[L].A_col[q2]) return false;
-  const int cand_ms[2] = {T > 1 ? m[1] - m[0] : 1, 0};
-  for (int t = 0; t < (T > 1 ? 1 : 2); ++t) {
-    bool ok = true;
-    for (int L = 0; L < T; ++L) ok = ok && (m[L] == m[0] + cand_ms[t] * L);
-    if (ok && apply_banded_available(T, m[0], cand_ms[t], c->w0)) { *m0 = m[0]; *ms = cand_ms[t]; return true; }
+      }
+    order[L] = L;
   }
-  return false;
+  std::sort(order, order + T, [&](int x, int y) { return reach[x] < reach[y] || (reach[x] == reach[y] && x < y); });
+  int shapes[64][4];
+  const int ns = apply_banded_shapes(shapes, 64);
+  long long best = -1;
+  for (int s = 0; s < ns; ++s) {
+    const int Tt = shapes[s][0], m0 = shapes[s][1], ms = shapes[s][2], W = shapes[s][3];
+    if (W < maxw || Tt < T || (T > 0 && Tt == 0) || (T == 0 && Tt != 0)) continue;
+    if (!apply_banded_available(0, 0, 0, W)) continue;           // the S-only apply needs the T = 0 kernel of the same width
+    int slot_of[TDDE_MAX_TERMS], next = 0;
+    bool ok = true;
+    for (int i = 0; i < T && ok; ++i) {                          // slots and terms both ascending in reach: greedy is optimal
+      while (next < Tt && m0 + ms * next < reach[order[i]]) ++next;
+      if (next >= Tt) ok = false; else slot_of[order[i]] = next++;
+    }
+    if (!ok) continue;
+    long long cost = 2 * W + 1;
+    for (int L = 0; L < Tt; ++L) cost += 2 * W + 1 + 2 * (m0 + ms * L);
+    if (best < 0 || cost < best) {
+      best = cost;
+      f->T = Tt; f->m0 = m0; f->ms = ms; f->W = W;
+      for (int L = 0; L < T; ++L) f->slot_of[L] = slot_of[L];
+    }
+  }
+  return best >= 0;
 }
 
 }  // namespace
@@ -127,8 +144,26 @@ extern "C" void tdde_destroy(tdde_handle* h) {
 
 static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H0_band, const int32_t* cls_of_chan,
                        const tdde_term* terms) {
-  const tdde_config& c = h->cfg;
   cudaStream_t s = h->stream;
+  // ---- which apply kernel (by the structure of the A_L) ----
+  h->user_terms = h->cfg.n_terms;
+  for (int L = 0; L < TDDE_MAX_TERMS; ++L) h->term_slot[L] = L;
+  BandFit fit;
+  h->path = fit_banded(&h->cfg, terms, &fit) ? 1 : 0;
+  if (const char* env = std::getenv("TDDE_APPLY_PATH")) { if (std::atoi(env) != 1) h->path = 0; }   // tests: force a lower tier
+  // banded path: re-slot the terms into the fitted shape; empty slots become zero terms (R = 0, A empty, g = 0)
+  std::vector<tdde_term> slotted;
+  std::vector<zc> zero_band((size_t)h->cfg.n_rad * 3, zc(0, 0));
+  std::vector<int32_t> zero_rowptr((size_t)h->cfg.n_ang + 1, 0);
+  if (h->path == 1) {
+    slotted.assign(std::max(fit.T, 1), tdde_term{1, 0, reinterpret_cast<const tdde_c64*>(zero_band.data()), zero_rowptr.data(), nullptr, nullptr});
+    for (int L = 0; L < h->user_terms; ++L) { slotted[fit.slot_of[L]] = terms[L]; h->term_slot[L] = fit.slot_of[L]; }
+    h->g_identity = fit.T == h->user_terms;
+    for (int L = 0; L < h->user_terms; ++L) h->g_identity = h->g_identity && fit.slot_of[L] == L;
+    h->cfg.n_terms = fit.T;
+    terms = slotted.data();
+  }
+  const tdde_config& c = h->cfg;
   const int n_rad = c.n_rad, w0 = c.w0, nd0 = 2 * w0 + 1, T = c.n_terms;
   h->ld = (c.n_ang + 31) / 32 * 32;
   h->nint = (long long)n_rad * h->ld;
@@ -137,10 +172,8 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
 
   CU(cudaGetDevice(&h->device));
   CU(cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device));
-  int m0 = 0, ms = 0;
-  h->path = detect_banded(&c, terms, &m0, &ms) ? 1 : 0;
-  if (const char* env = std::getenv("TDDE_APPLY_PATH")) { if (std::atoi(env) != 1) h->path = 0; }   // tests: force a lower tier
-  h->bT = T; h->bM0 = m0; h->bMS = ms; h->bW = w0;
+  const int m0 = h->path == 1 ? fit.m0 : 0, ms = h->path == 1 ? fit.ms : 0;
+  h->bT = T; h->bM0 = m0; h->bMS = ms; h->bW = h->path == 1 ? fit.W : w0;
   // Term split over two warp groups (256-thread CTA, one per SM, 255 registers each): measured on B200 it wins once
   // the per-thread A_L registers no longer fit (HBM-scale, T = 7: 3.21 -> 2.39 ms) and loses below (Large, T = 5:
   // 0.31 -> 0.37 ms), so it is chosen by the number of terms.
@@ -200,7 +233,7 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     }
   }
   h->norm_banded = (h->path != 0);
-  const int wpad = h->path == 2 ? h->spW : w0;             // half-width of the column bands the apply kernels read
+  const int wpad = h->path == 2 ? h->spW : h->bW;          // half-width of the column bands the apply kernels read
   const int ndp = 2 * wpad + 1;
   h->blk_count = (long long)c.n_cls * n_rad * ndp;
 

@@ -9,6 +9,7 @@
 #include <algorithm>
 #include <cstdlib>
 #include <cstring>
+#include <vector>
 #include "tdde_handle.h"
 
 static const cplx* blk_ptr(const tdde_handle* h, int blk) {
@@ -48,7 +49,7 @@ int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int b
     a.blk = blk_ptr(h, blk);
     a.Rall = h->d_Rall; a.slot = h->d_slot; a.cta_cls = h->d_cta_cls;
     a.Aoff = h->d_Aoff;
-    rc = launch_apply_banded(a, T, h->bM0, h->bMS, h->cfg.w0, h->apply_ng, h->stream);
+    rc = launch_apply_banded(a, T, h->bM0, h->bMS, h->bW, h->apply_ng, h->stream);
   } else if (h->path == 2) {
     a.blk = blk_ptr(h, blk);
     a.Rall = h->d_Rall; a.slot = h->d_slot; a.cta_cls = h->d_cta_cls;
@@ -110,6 +111,15 @@ static PrecArgs make_prec_args(tdde_handle* h, const cplx* x, cplx* y, const Sol
   p.aslot = h->d_slot; p.cta_cls = h->d_cta_cls;
   p.spikes_done = 0;
   return p;
+}
+
+const double* map_g(const tdde_handle* h, const double* g, long long rows, std::vector<double>& buf) {
+  if (h->g_identity || !g) return g;
+  const int Tu = h->user_terms, Ti = h->cfg.n_terms;
+  buf.assign((size_t)rows * Ti, 0.0);
+  for (long long r = 0; r < rows; ++r)
+    for (int L = 0; L < Tu; ++L) buf[(size_t)r * Ti + h->term_slot[L]] = g[(size_t)r * Tu + L];
+  return buf.data();
 }
 
 VecArgs make_vec_args(tdde_handle* h, SolverState* st, int fin) {
@@ -267,8 +277,10 @@ static int run_steps(tdde_handle* h, long long n_steps) {
 }
 
 extern "C" int tdde_propagate(tdde_handle* h, tdde_c64* c_dev, int64_t n_steps, const double* g_table, tdde_stats* st) {
-  if (!h || !c_dev || n_steps < 0 || (n_steps > 0 && h->cfg.n_terms > 0 && !g_table)) return TDDE_EINVAL;
+  if (!h || !c_dev || n_steps < 0 || (n_steps > 0 && h->user_terms > 0 && !g_table)) return TDDE_EINVAL;
   DeviceGuard dg(h->device);
+  std::vector<double> gbuf;
+  g_table = map_g(h, g_table, n_steps, gbuf);
   if (st) std::memset(st, 0, sizeof(*st));
   if (n_steps == 0) return 0;
   int rc;
@@ -303,8 +315,10 @@ extern "C" int tdde_propagate_host(tdde_handle* h, tdde_c64* c_host, int64_t n_s
 
 #ifdef TDDE_WITH_BENCH
 extern "C" int tdde_step_forced(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, int32_t n_iters, tdde_c64* trace_dev) {
-  if (!h || !c_dev || n_iters < 0 || (h->cfg.n_terms > 0 && !g_mid)) return TDDE_EINVAL;
+  if (!h || !c_dev || n_iters < 0 || (h->user_terms > 0 && !g_mid)) return TDDE_EINVAL;
   DeviceGuard dg(h->device);
+  std::vector<double> gbuf;
+  g_mid = map_g(h, g_mid, 1, gbuf);
   int rc;
   if ((rc = upload_g(h, g_mid, 1))) return rc;
   h->h_st->status = 0; h->h_st->stalled = 0; h->h_st->done = 1;
@@ -347,8 +361,10 @@ extern "C" int tdde_norm(tdde_handle* h, const tdde_c64* c_dev, double* out) {
 }
 
 extern "C" int tdde_apply(tdde_handle* h, tdde_c64 alpha, tdde_c64 beta, const double* g, const tdde_c64* x_dev, tdde_c64* y_dev) {
-  if (!h || !x_dev || !y_dev || x_dev == y_dev || (h->cfg.n_terms > 0 && !g)) return TDDE_EINVAL;
+  if (!h || !x_dev || !y_dev || x_dev == y_dev || (h->user_terms > 0 && !g)) return TDDE_EINVAL;
   DeviceGuard dg(h->device);
+  std::vector<double> gbuf;
+  g = map_g(h, g, 1, gbuf);
   int rc;
   if (h->cfg.n_terms > 0)
     CU(cudaMemcpyAsync(h->d_g_small, g, h->cfg.n_terms * sizeof(double), cudaMemcpyHostToDevice, h->stream));

@@ -25,6 +25,12 @@ struct tdde_handle {
   int* d_spcol = nullptr;
   bool use_subst = true;         // banded path: in-iteration applies use A y = p + i tau (coupling) y (needs a benign LU)
   int bT = 0, bM0 = 0, bMS = 0, bW = 0;
+  // The banded kernels are instantiated for a few (T, m_L, W) shapes; a problem whose structure FITS inside one (fewer terms, smaller
+  // offsets, narrower bands) runs on it with zero-filled slots: internally the handle then has cfg.n_terms = the shape's T, the
+  // caller's term L sits in slot term_slot[L], and every g the caller passes is expanded (map_g)
+  int user_terms = 0;
+  int term_slot[TDDE_MAX_TERMS] = {};
+  bool g_identity = true;
   int seg_len = 0;               // radial rows per thread (banded path)
   int seg_len_s = 0;             // radial rows per thread for the S-only (T = 0) apply: latency-bound, wants more CTAs
   int apply_ng = 1;              // warp groups the terms are split over (banded path)
@@ -120,3 +126,5 @@ int enqueue_precond(tdde_handle* h, const cplx* x, cplx* y, const SolverState* s
 int enqueue_vec_update(tdde_handle* h, int mode, SolverState* st, bool* fused);   // mode 0: p-update, 1: s-update (+ spike products when fused)
 VecArgs make_vec_args(tdde_handle* h, SolverState* st, int fin);
 int sync_state(tdde_handle* h);
+// g as the caller gives it ([rows][user_terms]) -> as the kernels index it ([rows][cfg.n_terms]); returns g itself when they coincide
+const double* map_g(const tdde_handle* h, const double* g, long long rows, std::vector<double>& buf);

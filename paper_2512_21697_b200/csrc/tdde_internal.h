@@ -175,6 +175,7 @@ int tdde_num_sms();   // multiprocessor count of the current device
 // launchers (each returns the number of kernels launched, or -1 if no instantiation fits)
 int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, int ng, cudaStream_t s);
 bool apply_banded_available(int T, int m0, int mstep, int W);
+int apply_banded_shapes(int (*out)[4], int cap);
 int launch_apply_generic(const ApplyArgs& a, int num_sms, cudaStream_t s);
 int launch_apply_sparse(const ApplyArgs& a, int W, cudaStream_t s);
 size_t apply_sparse_smem(int W, int T, int nslots, int xw, bool a_in_smem);

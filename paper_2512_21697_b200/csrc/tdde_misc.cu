@@ -26,8 +26,10 @@ extern "C" int64_t tdde_launch_count(const tdde_handle* h) { return h ? h->launc
 
 extern "C" int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, const double* g, double* ms_out) {
   if (!h || !ms_out || reps <= 0 || which < 0 || which > 6) return TDDE_EINVAL;
-  if (which == 0 && h->cfg.n_terms > 0 && !g) return TDDE_EINVAL;
+  if (which == 0 && h->user_terms > 0 && !g) return TDDE_EINVAL;
   DeviceGuard dg(h->device);
+  std::vector<double> gbuf;
+  g = map_g(h, g, 1, gbuf);
   cudaStream_t s = h->stream;
   SolverState* sb = h->d_st_bench;
   // finite, non-trivial data in every work vector

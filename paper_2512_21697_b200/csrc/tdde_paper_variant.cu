@@ -92,7 +92,8 @@ __global__ void __launch_bounds__(256) k_pv_spmv(PvArgs p, long long n, const cp
 
 extern "C" int tdde_paper_variant(tdde_handle* h, const double* g, const tdde_c64* x_dev, tdde_c64* y_dev, int32_t reps,
                                   double* ms_assemble, double* ms_spmv, int64_t* nnz_out) {
-  if (!h || !x_dev || !y_dev || reps <= 0 || (h->cfg.n_terms > 0 && !g)) return TDDE_EINVAL;
+  if (!h || !x_dev || !y_dev || reps <= 0 || (h->user_terms > 0 && !g)) return TDDE_EINVAL;
+  if (h->bW != h->cfg.w0 || !h->g_identity) return TDDE_EINVAL;      // only for problems that ARE an instantiated shape (no zero-filled slots)
   if (h->path != 1) return TDDE_EINVAL;                               // pattern known in closed form only there
   const int n_ang = h->cfg.n_ang, n_rad = h->cfg.n_rad, w = h->cfg.w0, T = h->cfg.n_terms;
   PvArgs p;

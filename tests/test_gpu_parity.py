@@ -525,14 +525,16 @@ def test_no_coupling_terms(bw):
     prop.close()
 
 
-@pytest.mark.parametrize("bw,T", [(9, 3), (11, 4), (15, 6), (5, 2)])
+@pytest.mark.parametrize("bw,T", [(9, 3), (11, 4), (15, 6), (5, 2), (7, 6), (13, 1)])
 def test_untemplated_bandwidths_and_term_counts(bw, T):
-    """Half-bandwidths outside {3, 6, 9, 13} (w = 4, 5, 7, 2) and T = 4, 6: whatever kernels the library picks for them,
-    apply, preconditioner and propagation must match the oracle."""
+    """Half-bandwidths outside {3, 6, 9, 13} (w = 4, 5, 7, 2) and T = 1, 4, 6: banded couplings that are not one of the instantiated
+    shapes FIT inside one (zero-filled slots, padded bands) and stay on the register-resident kernel; apply, preconditioner and
+    propagation must match the oracle."""
     from paper_2512_21697_b200 import Tdde
     p = tdde_inputs.make_synthetic(name="odd", n_ang=75, n_r=33, bandwidth=bw, n_terms=T, dt=0.005, n_steps=3, rtol=1e-10,
                                    seed=bw, phase=np.pi / 2, e0=2.0)
     prop = Tdde(p)
+    assert prop.apply_path == "banded"
     ops, fact = orc.assemble(p), orc.factor_precond(p)
     x = rand_vec(p.n, 6)
     g = np.linspace(0.4, 1.3, T)
@@ -544,6 +546,43 @@ def test_untemplated_bandwidths_and_term_counts(bw, T):
     c = prop.to_device(p.c0)
     st = prop.propagate(c, p.g_table(p.n_steps))
     assert st["steps"] == p.n_steps and rel(c.cpu().numpy(), c_ref) <= 1e-9
+    prop.close()
+
+
+def test_banded_fit_with_permuted_and_thinned_terms():
+    """Terms given in an order that is not ascending in reach, with some offsets missing and per-term bandwidths below w0: the
+    structure fit re-slots them into an instantiated shape; g is given per caller term and must follow its term."""
+    from paper_2512_21697_b200 import Tdde
+    base = tdde_inputs.make_synthetic(name="perm", n_ang=140, n_r=31, bandwidth=13, n_terms=5, dt=0.005, n_steps=3, rtol=1e-10, seed=14,
+                                      phase=np.pi / 2, e0=2.0)
+    rng = np.random.default_rng(3)
+    order = [3, 0, 4, 1]                                         # four of the five terms, shuffled (reaches 4, 1, 5, 2)
+    terms = []
+    for L in order:
+        t = base.terms[L]
+        keep = np.ones(len(t.A_col), dtype=bool)
+        rows = np.repeat(np.arange(base.n_ang), np.diff(t.A_rowptr))
+        keep &= ~((np.abs(t.A_col - rows) == 2) & (L == 3))      # drop the offsets +-2 of the reach-4 term (stays Hermitian)
+        rowptr = np.concatenate([[0], np.cumsum(np.bincount(rows[keep], minlength=base.n_ang))]).astype(np.int32)
+        w = 6 if L != 0 else 4                                   # one term with a narrower radial band
+        R = t.R_band if w == 6 else np.ascontiguousarray(t.R_band[:, 2:-2])
+        terms.append(tdde_inputs.Term(w=w, R_band=R, A_rowptr=rowptr, A_col=t.A_col[keep], A_val=t.A_val[keep]))
+    amps = np.array([0.7, -1.3, 0.4, 2.1])
+    d = dict(base.__dict__)
+    d.update(terms=terms, g_of_t=lambda t, _a=amps: _a * np.cos(0.057 * t))
+    p = tdde_inputs.Problem(**d)
+    prop = Tdde(p)
+    assert prop.apply_path == "banded"
+    ops, fact = orc.assemble(p), orc.factor_precond(p)
+    x = rand_vec(p.n, 6)
+    for g in (amps, np.array([1.0, 0.0, 0.0, 0.0]), np.array([0.0, 0.0, 1.0, 0.0])):
+        y = prop.apply(1.0, 0.5j * p.dt, g, prop.to_device(x)).cpu().numpy()
+        assert rel(y, orc.apply(ops, 1.0, 0.5j * p.dt, g, x)) <= 1e-12, g
+    c_ref, infos = orc.propagate(p, ops, fact, p.c0, 3)
+    c = prop.to_device(p.c0)
+    st = prop.propagate(c, p.g_table(3))
+    assert st["steps"] == 3 and rel(c.cpu().numpy(), c_ref) <= 1e-9
+    tr = prop.step_forced(prop.to_device(p.c0), p.g_mid(0), 1, trace=False)
     prop.close()
 
 
@@ -607,6 +646,7 @@ def test_generic_fallback_path_and_bounded_grid(monkeypatch):
     parity, and a shape with more (row, channel-block) work items than reduction slots (70400 > 65536)."""
     from paper_2512_21697_b200 import Tdde
     monkeypatch.setenv("TDDE_NO_STAGED", "1")
+    monkeypatch.setenv("TDDE_APPLY_PATH", "0")
     p = _random_sparse_problem(43, n_ang=60, n_r=25, bandwidths=[4, 6], nnz_row=3)
     prop = Tdde(p)
     assert prop.apply_path == "generic"
