@@ -15,6 +15,14 @@ extern "C" {
  * vectors p, v, s, t, x, r, y, z (this order, boundary layout).  Synchronises. */
 int tdde_step_forced(tdde_handle* h, tdde_c64* c_dev, const double* g_mid, int32_t n_iters, tdde_c64* trace_dev);
 
+/* Test export of the kernel an iteration uses for v = A y on the banded path (R21): y = addv + beta sum_L g[L] (A_L (x) R_L) x
+ * with the fused sums dots[0..1] = <aux, y> (re, im), dots[2] = ||y||^2 over all n elements (aux_dev nullable: dots[0..1] = 0).
+ * which: 0 = the kernel the handle would use (DMMA variant when the shape has one), 1 = force the register-window kernel.
+ * x_dev, addv_dev, aux_dev, y_dev: device, n complex128, boundary layout, y must not alias the inputs; dots: host [3], nullable.
+ * TDDE_EINVAL when the handle is not on the banded path (tdde_apply_path != 1) or has no terms.  Synchronises. */
+int tdde_apply_coupling(tdde_handle* h, tdde_c64 beta, const double* g, const tdde_c64* x_dev, const tdde_c64* addv_dev,
+                        const tdde_c64* aux_dev, tdde_c64* y_dev, int32_t which, double* dots);
+
 /* Measurement helpers (timed in bench.py; no effect on state).
  *   tdde_time_kernel: enqueue `reps` launches of one internal kernel on the handle's stream between two CUDA
  *   events and return the mean milliseconds per launch in *ms_out.  which: 0 = operator apply v = A y with

@@ -18,7 +18,7 @@ LIB_PATH = os.environ.get("TDDE_LIB_PATH", os.path.join(_HERE, "libtdde.so"))
 
 EXPORTS = [
     "tdde_create", "tdde_step", "tdde_propagate", "tdde_norm", "tdde_apply", "tdde_precond",
-    "tdde_propagate_host", "tdde_step_forced", "tdde_time_kernel", "tdde_fp64_peak", "tdde_launch_count",
+    "tdde_propagate_host", "tdde_step_forced", "tdde_apply_coupling", "tdde_time_kernel", "tdde_fp64_peak", "tdde_launch_count",
     "tdde_apply_path", "tdde_set_eigenstates", "tdde_project", "tdde_eigensolve", "tdde_selftest_partition", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
 ]
 
@@ -77,6 +77,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.tdde_precond.argtypes = [vp, vp, vp]
     lib.tdde_step_forced.argtypes = [vp, vp, vp, i32, vp]
     lib.tdde_time_kernel.argtypes = [vp, i32, i32, vp, C.POINTER(dbl)]
+    lib.tdde_apply_coupling.argtypes = [vp, tdde_c64, vp, vp, vp, vp, vp, i32, vp]
+    lib.tdde_apply_coupling.restype = C.c_int
     lib.tdde_fp64_peak.argtypes = [vp, C.POINTER(dbl)]
     lib.tdde_launch_count.argtypes = [vp]
     lib.tdde_launch_count.restype = i64
@@ -230,6 +232,17 @@ class Tdde:
                                  self._vec(x_dev, "x"), self._vec(y, "y"))
         _check(self.lib, rc, "tdde_apply")
         return y
+
+    def apply_coupling(self, beta: complex, g, x_dev, addv_dev, aux_dev=None, which: int = 0):
+        """y = addv + beta sum_L g_L (A_L (x) R_L) x by the in-iteration kernel; returns (y, <aux,y>, ||y||^2)  (tdde_apply_coupling)."""
+        g = _g_array(g, self.n_terms)
+        y = self.torch.empty_like(x_dev)
+        b = complex(beta)
+        dots = np.zeros(3)
+        rc = self.lib.tdde_apply_coupling(self.h, tdde_c64(b.real, b.imag), _np_ptr(g), self._vec(x_dev, "x"), self._vec(addv_dev, "addv"),
+                                          self._vec(aux_dev, "aux") if aux_dev is not None else None, self._vec(y, "y"), int(which), _np_ptr(dots))
+        _check(self.lib, rc, "tdde_apply_coupling")
+        return y, complex(dots[0], dots[1]), float(dots[2])
 
     def precond(self, x_dev, y_dev=None):
         y = self.torch.empty_like(x_dev) if y_dev is None else y_dev

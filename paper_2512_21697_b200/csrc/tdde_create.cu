@@ -125,7 +125,7 @@ extern "C" void tdde_destroy(tdde_handle* h) {
   if (!h) return;
   DeviceGuard dg(h->device);
   cudaStreamSynchronize(h->stream);
-  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_slot, h->d_cta_cls, h->d_eig, h->d_proj, h->d_pslot, h->d_warp_cls, h->d_spval, h->d_spcol, h->d_Wsp, h->d_Corner, h->d_Schur, h->d_rsm, h->d_rsp, h->d_Lcol, h->d_Ucol, h->X, h->r,
+  void* ptrs[] = {h->d_cls, h->d_S, h->d_H0, h->d_Mp, h->d_blk_tmp, h->d_Aoff, h->d_Rall, h->d_Rfrag, h->d_slot, h->d_cta_cls, h->d_eig, h->d_proj, h->d_pslot, h->d_warp_cls, h->d_spval, h->d_spcol, h->d_Wsp, h->d_Corner, h->d_Schur, h->d_rsm, h->d_rsp, h->d_Lcol, h->d_Ucol, h->X, h->r,
                   h->rhat, h->p, h->v, h->s, h->t, h->y, h->z, h->c_stage, h->d_st, h->d_st_bench, h->d_partials,
                   h->d_ticket, h->d_g, h->d_g_small, h->d_zero_g};
   for (void* p : ptrs) if (p) cudaFree(p);
@@ -411,6 +411,25 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
         std::memcpy(&Rall[((size_t)j * T + L) * ndp], &Rc[(size_t)j * ndp], ndp * sizeof(zc));
     }
     if ((rc = dev_upload(&h->d_Rall, reinterpret_cast<cplx*>(Rall.data()), Rall.size(), s))) return rc;
+    // DMMA variant of the in-iteration apply (tdde_apply_mma.cu): fragment table + its own segment length (64-channel CTAs,
+    // one per SM, rows in multiples of 8)
+    if (h->path == 1 && T > 0 && apply_mma_available(T, h->bM0, h->bMS, h->bW) && !std::getenv("TDDE_NO_MMA")) {
+      std::vector<double> frags;
+      if (build_mma_frags(T, h->bW, n_rad, Rall.data(), frags)) {
+        if ((rc = dev_upload(&h->d_Rfrag, frags.data(), frags.size(), s))) return rc;
+        const int nc = apply_mma_channels(), chan_blocks = (h->ld + nc - 1) / nc, halo = apply_mma_halo(h->bW);
+        long long best_cost = -1;
+        int best_seg = (n_rad + 7) / 8 * 8;
+        for (int seg = 8; seg <= (n_rad + 7) / 8 * 8; seg += 8) {
+          const long long ctas = (long long)chan_blocks * ((n_rad + seg - 1) / seg);
+          const long long waves = (ctas + h->num_sms - 1) / h->num_sms;
+          const long long cost = waves * (seg + halo);
+          if (best_cost < 0 || cost < best_cost) { best_cost = cost; best_seg = seg; }
+        }
+        h->seg_len_m = best_seg;
+        if (const char* env = std::getenv("TDDE_MMA_SEG")) h->seg_len_m = std::max(8, std::atoi(env) / 8 * 8);
+      }
+    }
     if (h->path == 2) {
       if ((rc = dev_upload(&h->d_spval, reinterpret_cast<cplx*>(ell_val.data()), ell_val.size(), s))) return rc;
       if ((rc = dev_upload(&h->d_spcol, ell_col.data(), ell_col.size(), s))) return rc;

@@ -49,7 +49,14 @@ int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int b
     a.blk = blk_ptr(h, blk);
     a.Rall = h->d_Rall; a.slot = h->d_slot; a.cta_cls = h->d_cta_cls;
     a.Aoff = h->d_Aoff;
-    rc = launch_apply_banded(a, T, h->bM0, h->bMS, h->bW, h->apply_ng, h->stream);
+    rc = -1;
+    if (a.addv && T > 0 && emode == 0 && h->seg_len_m > 0) {      // in-iteration apply: DMMA variant
+      a.Rfrag = h->d_Rfrag;
+      a.seg_len = h->seg_len_m;
+      rc = launch_apply_mma(a, T, h->bM0, h->bMS, h->bW, h->stream);
+      if (rc == -1) a.seg_len = h->seg_len;
+    }
+    if (rc == -1) rc = launch_apply_banded(a, T, h->bM0, h->bMS, h->bW, h->apply_ng, h->stream);
   } else if (h->path == 2) {
     a.blk = blk_ptr(h, blk);
     a.Rall = h->d_Rall; a.slot = h->d_slot; a.cta_cls = h->d_cta_cls;

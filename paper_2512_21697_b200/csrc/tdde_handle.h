@@ -32,6 +32,8 @@ struct tdde_handle {
   int term_slot[TDDE_MAX_TERMS] = {};
   bool g_identity = true;
   int seg_len = 0;               // radial rows per thread (banded path)
+  int seg_len_m = 0;             // radial rows per CTA of the DMMA apply (multiple of 8); 0 = that kernel is not used
+  double* d_Rfrag = nullptr;     // its B-operand fragment table
   int seg_len_s = 0;             // radial rows per thread for the S-only (T = 0) apply: latency-bound, wants more CTAs
   int apply_ng = 1;              // warp groups the terms are split over (banded path)
   bool norm_banded = false;      // S-only apply can use the banded T=0 kernel
@@ -127,4 +129,5 @@ int enqueue_vec_update(tdde_handle* h, int mode, SolverState* st, bool* fused); 
 VecArgs make_vec_args(tdde_handle* h, SolverState* st, int fin);
 int sync_state(tdde_handle* h);
 // g as the caller gives it ([rows][user_terms]) -> as the kernels index it ([rows][cfg.n_terms]); returns g itself when they coincide
+bool build_mma_frags(int T, int W, int n_rad, const void* Rall, std::vector<double>& out);   // tdde_apply_mma.cu
 const double* map_g(const tdde_handle* h, const double* g, long long rows, std::vector<double>& buf);

@@ -79,7 +79,8 @@ enum FinCode {
   FIN_S,       // d1 = ||s||^2 -> half-step exit test
   FIN_R,       // d0 = <rhat, r>, d1 = ||r||^2 -> convergence test, rho, beta
   FIN_RES0,    // d1 = ||r0||^2 (start of step, from the H-apply that writes r0 and rhat): res2 = d1
-  FIN_R0S      // d1 = ||b||^2 (start of step, from the S-apply): the FIN_R0 logic with ||r0||^2 taken from res2
+  FIN_R0S,     // d1 = ||b||^2 (start of step, from the S-apply): the FIN_R0 logic with ||r0||^2 taken from res2
+  FIN_DOTS     // test export: rho_old = d0, res2 = d1, nothing else
 };
 
 struct ReduceCtx {
@@ -113,6 +114,7 @@ struct ApplyArgs {
   const int* slot;         // [ld] index of the channel's class in its CTA's class list, -1 = not staged
   const int* cta_cls;      // [n_cta][TDDE_AP_MAXC] classes staged per CTA (-1 = unused)
   const cplx* Aoff;        // banded path: [n_slots][ld], slot = (term, offset) in kernel order
+  const double* Rfrag;     // DMMA path (tdde_apply_mma.cu): B-operand fragments of every 4-row slice, nullable
   // staged sparse-A path (tdde_apply_sparse.cu): ELL rows of every term, slot-major [sp_nslots][ld]; blk and Rall padded to 2W+1
   const cplx* sp_val;
   const int* sp_col;       // absolute internal channel index (own channel for padding slots)
@@ -177,6 +179,11 @@ int launch_apply_banded(const ApplyArgs& a, int T, int m0, int mstep, int W, int
 bool apply_banded_available(int T, int m0, int mstep, int W);
 int apply_banded_shapes(int (*out)[4], int cap);
 int launch_apply_generic(const ApplyArgs& a, int num_sms, cudaStream_t s);
+// DMMA variant of the in-iteration banded apply (y = addv + coupling terms): shapes, fragment table, launcher
+bool apply_mma_available(int T, int m0, int mstep, int W);
+int apply_mma_halo(int W);
+int apply_mma_channels();
+int launch_apply_mma(const ApplyArgs& a, int T, int m0, int mstep, int W, cudaStream_t s);
 int launch_apply_sparse(const ApplyArgs& a, int W, cudaStream_t s);
 size_t apply_sparse_smem(int W, int T, int nslots, int xw, bool a_in_smem);
 int launch_precond(const PrecArgs& a, cudaStream_t s);

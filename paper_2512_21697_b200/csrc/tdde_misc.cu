@@ -74,6 +74,35 @@ extern "C" int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, con
   return rc;
 }
 
+extern "C" int tdde_apply_coupling(tdde_handle* h, tdde_c64 beta, const double* g, const tdde_c64* x_dev, const tdde_c64* addv_dev,
+                                   const tdde_c64* aux_dev, tdde_c64* y_dev, int32_t which, double* dots) {
+  if (!h || !g || !x_dev || !addv_dev || !y_dev || y_dev == x_dev || y_dev == addv_dev || y_dev == aux_dev) return TDDE_EINVAL;
+  if (h->path != 1 || h->cfg.n_terms == 0 || !h->use_subst) return TDDE_EINVAL;
+  DeviceGuard dg(h->device);
+  std::vector<double> gbuf;
+  g = map_g(h, g, 1, gbuf);
+  cudaStream_t s = h->stream;
+  CU(cudaMemcpyAsync(h->d_g_small, g, h->cfg.n_terms * sizeof(double), cudaMemcpyHostToDevice, s));
+  h->launches += launch_to_internal(reinterpret_cast<const cplx*>(x_dev), h->y, h->cfg.n_ang, h->cfg.n_rad, h->ld, s);
+  h->launches += launch_to_internal(reinterpret_cast<const cplx*>(addv_dev), h->p, h->cfg.n_ang, h->cfg.n_rad, h->ld, s);
+  if (aux_dev) h->launches += launch_to_internal(reinterpret_cast<const cplx*>(aux_dev), h->rhat, h->cfg.n_ang, h->cfg.n_rad, h->ld, s);
+  // FIN_DOTS parks the raw sums in the (never-idle) bench state
+  const int keep = h->seg_len_m;
+  if (which == 1) h->seg_len_m = 0;
+  SolverState* sb = h->d_st_bench;
+  int rc = enqueue_apply(h, h->y, h->v, aux_dev ? h->rhat : nullptr, BLK_MP, make_double2(beta.re, beta.im), true, h->d_g_small, nullptr, 0,
+                         FIN_DOTS, sb, h->p);
+  h->seg_len_m = keep;
+  if (rc) return rc;
+  h->launches += launch_to_boundary(h->v, reinterpret_cast<cplx*>(y_dev), h->cfg.n_ang, h->cfg.n_rad, h->ld, s);
+  SolverState hs;
+  CU(cudaMemcpyAsync(&hs, sb, sizeof(SolverState), cudaMemcpyDeviceToHost, s));
+  CU(cudaStreamSynchronize(s));
+  if (dots) { dots[0] = hs.rho_old.x; dots[1] = hs.rho_old.y; dots[2] = hs.res2; }
+  CU(cudaGetLastError());
+  return 0;
+}
+
 extern "C" int tdde_fp64_peak(void* cuda_stream, double* flops_out) {
   if (!flops_out) return TDDE_EINVAL;
   cudaStream_t s = (cudaStream_t)cuda_stream;

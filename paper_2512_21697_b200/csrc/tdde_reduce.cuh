@@ -59,6 +59,7 @@ __device__ inline void finalize_scalars(SolverState* st, int fin, double d0x, do
   switch (fin) {
     case FIN_NB: st->nb2 = d1; break;
     case FIN_NORM: st->norm_out = d0x; break;
+    case FIN_DOTS: st->rho_old = make_double2(d0x, d0y); st->res2 = d1; break;
     case FIN_RES0: st->res2 = d1; break;
     case FIN_R0S:
       d0x = d1;                                  // ||b||^2 from this kernel, ||r0||^2 from the previous one

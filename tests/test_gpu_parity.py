@@ -808,3 +808,55 @@ def test_device_eigensolve_next4(hyd):
     assert np.max(np.abs(Eq - Eq_ref)) <= 1e-12 * np.max(np.abs(Eq_ref))
     S, H = tdde_inputs.band_to_dense(q.S_band[2]), tdde_inputs.band_to_dense(q.H0_band[2])
     assert np.linalg.norm(H @ Vq[2].T - (S @ Vq[2].T) * Eq[2][None, :]) <= 1e-12 * np.linalg.norm(H) * 45
+
+
+# ---- in-iteration apply (R21 / 4.1): y = addv + beta sum_L g_L (A_L (x) R_L) x, DMMA variant and register-window variant ----
+@pytest.mark.parametrize("n_ang,n_r,T,bw,seg", [(257, 53, 7, 13, 0), (100, 41, 7, 19, 16), (130, 37, 5, 13, 8), (96, 64, 7, 13, 24),
+                                                (33, 9, 7, 13, 0)])
+def test_coupling_apply_parity_mma_and_window(n_ang, n_r, T, bw, seg, monkeypatch):
+    """All outputs and the fused sums of the kernel an iteration uses for v = A y, against the oracle's coupling part
+    (apply with g minus apply with g = 0), for the DMMA kernel (which=0) and the register-window kernel (which=1): channel counts
+    that are not multiples of 8 / 96, radial sizes that are not multiples of 8, several radial segments (TDDE_MMA_SEG)."""
+    from paper_2512_21697_b200 import Tdde
+    if seg:
+        monkeypatch.setenv("TDDE_MMA_SEG", str(seg))
+    p = tdde_inputs.make_synthetic(n_ang=n_ang, n_r=n_r, bandwidth=bw, n_terms=T, dt=0.01, n_steps=1, rtol=1e-10, seed=n_ang + T,
+                                   name="coupling")
+    prop = Tdde(p)
+    assert prop.apply_path == "banded"
+    ops = orc.assemble(p)
+    x, addv, aux = rand_vec(p.n, 11), rand_vec(p.n, 12), rand_vec(p.n, 13)
+    g = np.linspace(0.4, 1.7, T)
+    beta = 0.3 - 0.8j
+    y_ref = addv + orc.apply(ops, 0.0, beta, g, x) - orc.apply(ops, 0.0, beta, np.zeros(T), x)
+    for which in (0, 1):
+        y, dot, nrm2 = prop.apply_coupling(beta, g, prop.to_device(x), prop.to_device(addv), prop.to_device(aux), which=which)
+        y = y.cpu().numpy()
+        assert rel(y, y_ref) <= 1e-12, (which, n_ang, n_r, T, bw)
+        assert np.max(np.abs(y - y_ref)) <= 1e-12 * np.sqrt(np.mean(np.abs(y_ref) ** 2)) * 50, which
+        assert abs(dot - np.vdot(aux, y_ref)) <= 1e-12 * np.linalg.norm(aux) * np.linalg.norm(y_ref), which
+        assert abs(nrm2 - np.vdot(y_ref, y_ref).real) <= 1e-12 * np.vdot(y_ref, y_ref).real, which
+    prop.close()
+
+
+def test_mma_and_window_propagation_agree(monkeypatch):
+    """Same propagation with the DMMA kernel and with TDDE_NO_MMA=1: same iteration counts, states equal to rounding, both within
+    1e-9 of the oracle."""
+    from paper_2512_21697_b200 import Tdde
+    p = tdde_inputs.make_synthetic(n_ang=200, n_r=45, bandwidth=13, n_terms=7, dt=0.01, n_steps=4, rtol=1e-10, seed=77, name="mma_prop",
+                                   phase=np.pi / 2, e0=2.0)
+    ops, fact = orc.assemble(p), orc.factor_precond(p)
+    c_ref, infos = orc.propagate(p, ops, fact, p.c0, 4)
+    out = []
+    for no_mma in (False, True):
+        if no_mma:
+            monkeypatch.setenv("TDDE_NO_MMA", "1")
+        prop = Tdde(p)
+        c = prop.to_device(p.c0)
+        st = prop.propagate(c, p.g_table(4))
+        out.append((c.cpu().numpy(), st["half_iters"]))
+        prop.close()
+    assert out[0][1] == out[1][1]
+    assert rel(out[0][0], out[1][0]) <= 1e-13
+    assert rel(out[0][0], c_ref) <= 1e-9 and rel(out[1][0], c_ref) <= 1e-9
+    assert abs(out[0][1] - sum(i.half_iters for i in infos)) <= 4
