@@ -347,8 +347,8 @@ def ours_main(args):
                                         "h2d_bytes_per_step": n * 16 + T * 8, "d2h_bytes_per_step": n * 16,
                                         "note": "K tdde_propagate_host calls of one step each"}},
             "roofline": {"bound": "alu",
-                         "kernel": ("k_apply_banded (v = A y = p + i tau (sum_L g_L A_L (x) R_L) y with fused <rhat,v>)" if subst else
-                                    "k_apply_%s (v = A y with fused <rhat,v>)" % ("sparse" if prop.apply_path == "staged" else prop.apply_path)),
+                         "kernel": (prop.iter_apply_kernel + " (v = A y = p + i tau (sum_L g_L A_L (x) R_L) y with fused <rhat,v>)" if subst else
+                                    prop.iter_apply_kernel + " (v = A y with fused <rhat,v>)"),
                          "achieved": ach, "peak": fp64_peak_nominal / 1e12, "unit": "TFLOP/s",
                          "frac": ach / (fp64_peak_nominal / 1e12), "traffic": traffic,
                          "algorithmic_bytes_per_launch": bytes_per["apply"] * nint,

@@ -47,6 +47,10 @@ int tdde_paper_variant(tdde_handle* h, const double* g, const tdde_c64* x_dev, t
  * partitions actually used (>= 1; the plan shrinks P until interiors are >= 8 w rows) or a negative tdde_status. */
 int tdde_selftest_partition(int32_t n, int32_t w, int32_t P, uint32_t seed, double* rel_res);
 
+/* Which kernel an iteration uses for v = A y: 0 = k_apply_generic, 1 = k_apply_banded (register window), 2 = k_apply_sparse (staged),
+ * 3 = k_apply_mma (banded path, radial contraction on the FP64 tensor-core path). */
+int tdde_iter_apply_kernel(const tdde_handle* h);
+
 /* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
 int64_t tdde_launch_count(const tdde_handle* h);
 

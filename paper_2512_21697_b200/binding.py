@@ -19,7 +19,7 @@ LIB_PATH = os.environ.get("TDDE_LIB_PATH", os.path.join(_HERE, "libtdde.so"))
 EXPORTS = [
     "tdde_create", "tdde_step", "tdde_propagate", "tdde_norm", "tdde_apply", "tdde_precond",
     "tdde_propagate_host", "tdde_step_forced", "tdde_apply_coupling", "tdde_time_kernel", "tdde_fp64_peak", "tdde_launch_count",
-    "tdde_apply_path", "tdde_set_eigenstates", "tdde_project", "tdde_eigensolve", "tdde_selftest_partition", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
+    "tdde_apply_path", "tdde_iter_apply_kernel", "tdde_set_eigenstates", "tdde_project", "tdde_eigensolve", "tdde_selftest_partition", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
 ]
 
 STATUS = {0: "TDDE_OK", -1: "TDDE_EINVAL", -2: "TDDE_ENOMEM", -3: "TDDE_ECUDA", -4: "TDDE_ESINGULAR",
@@ -83,6 +83,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.tdde_launch_count.argtypes = [vp]
     lib.tdde_launch_count.restype = i64
     lib.tdde_apply_path.argtypes = [vp]
+    lib.tdde_iter_apply_kernel.argtypes = [vp]
+    lib.tdde_iter_apply_kernel.restype = C.c_int
     lib.tdde_set_eigenstates.argtypes = [vp, i32, vp]
     lib.tdde_set_eigenstates.restype = C.c_int
     lib.tdde_project.argtypes = [vp, vp, vp]
@@ -299,6 +301,12 @@ class Tdde:
     @property
     def apply_path(self) -> str:
         return {1: "banded", 2: "staged", 0: "generic"}.get(self.lib.tdde_apply_path(self.h), "unknown")
+
+    @property
+    def iter_apply_kernel(self) -> str:
+        """The kernel an iteration uses for v = A y (tdde_iter_apply_kernel)."""
+        return {0: "k_apply_generic", 1: "k_apply_banded", 2: "k_apply_sparse", 3: "k_apply_mma"}.get(
+            self.lib.tdde_iter_apply_kernel(self.h), "unknown")
 
     def close(self):
         if getattr(self, "h", None):

@@ -225,7 +225,9 @@ __global__ void __launch_bounds__(MM_NT, 1) k_apply_mma(const __grid_constant__ 
       }
     }
   };
+#ifndef MM_NOPF
   prefetch(0);
+#endif
   __syncthreads();                                              // As visible to the whole warp
   cplx d0 = make_double2(0, 0);
   double d1 = 0;
@@ -287,6 +289,9 @@ __global__ void __launch_bounds__(MM_NT, 1) k_apply_mma(const __grid_constant__ 
   auto emit = [&](int u) {                                         // tile u - EV is complete: combine, add, store, inner products
     const int v = u - G::EV;
     if (v >= 0 && v < ntile) {
+#ifdef MM_NOPF
+      prefetch(v);
+#endif
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
         const int i = i0 + 8 * v + 2 * r + e;
@@ -304,7 +309,9 @@ __global__ void __launch_bounds__(MM_NT, 1) k_apply_mma(const __grid_constant__ 
       for (int e = 0; e < 3; ++e) { acc[k][e][0] = acc[k + 1][e][0]; acc[k][e][1] = acc[k + 1][e][1]; }
 #pragma unroll
     for (int e = 0; e < 3; ++e) { acc[NL - 1][e][0] = 0; acc[NL - 1][e][1] = 0; }
+#ifndef MM_NOPF
     if (v + 1 < ntile) prefetch(v + 1);
+#endif
   };
   using I0 = std::integral_constant<int, 0>;
   using I1 = std::integral_constant<int, 1>;

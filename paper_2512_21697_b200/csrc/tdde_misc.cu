@@ -20,6 +20,12 @@ extern "C" const char* tdde_strerror(int status) {
 extern "C" const char* tdde_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
 extern "C" int tdde_version(void) { return 2; }
 extern "C" int tdde_apply_path(const tdde_handle* h) { return h ? h->path : -1; }
+#ifdef TDDE_WITH_BENCH
+extern "C" int tdde_iter_apply_kernel(const tdde_handle* h) {
+  if (!h) return -1;
+  return (h->path == 1 && h->use_subst && h->cfg.n_terms > 0 && h->seg_len_m > 0) ? 3 : h->path;
+}
+#endif
 
 #ifdef TDDE_WITH_BENCH
 extern "C" int64_t tdde_launch_count(const tdde_handle* h) { return h ? h->launches : 0; }

@@ -20,6 +20,9 @@
 #include "tdde_reduce.cuh"
 
 #define PC_NT 32
+#ifndef TDDE_SCHUR_DEPTH
+#define TDDE_SCHUR_DEPTH(W) ((W) <= 8 ? 2 : 1)   // measured on B200: 3 and 4 sets spill and lose (HBM-scale solve 0.50 -> 0.56 / 0.60 ms)
+#endif
 #define PC_ROWS 8
 #ifndef PC_STAGES
 #define PC_STAGES 2
@@ -252,7 +255,7 @@ __global__ void __launch_bounds__(PC_NT* W, (W <= 6 ? 2 : 1)) k_precond_schur(co
   constexpr int WW = W * W;
   const cplx* Sk = p.Schur + (size_t)p.cls[a] * ns * 3 * WW + c * W;  // row c of every block
   auto sep_row = [&](int j) { return pc_lo(p, j) + pc_len(p, j) + c; };
-  constexpr bool PIPE = W <= 8;             // two operand sets of the forward pass are 2 (2 W + 3) complex registers
+  constexpr int D = TDDE_SCHUR_DEPTH(W);    // operand sets in flight: each is 2 W + 3 complex registers in the forward pass
   // ---------------- forward ----------------
   auto ffetch = [&](int j, SchurFwd<W>& o) {
     if (j >= ns) return;
@@ -282,20 +285,21 @@ __global__ void __launch_bounds__(PC_NT* W, (W <= 6 ? 2 : 1)) k_precond_schur(co
     }
     p.rsp[((size_t)j * W + c) * ld + a] = cadd(z0, z1);
   };
-  if (PIPE) {
-    SchurFwd<W> A, B;
-    ffetch(0, A);
-    for (int j = 0; j < ns; j += 2) {
-      ffetch(j + 1, B);
-      fstep(j, A);
-      if (j + 1 < ns) {
-        ffetch(j + 2, A);
-        fstep(j + 1, B);
+  // operands of step j + D - 1 are requested before step j runs: the chain is latency-bound (one block product and one CTA barrier
+  // per step), so the loads of D - 1 steps are in flight behind it
+  {
+    SchurFwd<W> buf[D];
+#pragma unroll
+    for (int k = 0; k < D - 1; ++k) ffetch(k, buf[k]);
+    for (int j = 0; j < ns; j += D) {
+#pragma unroll
+      for (int k = 0; k < D; ++k) {
+        if (j + k < ns) {
+          ffetch(j + k + D - 1, buf[(k + D - 1) % D]);
+          fstep(j + k, buf[k]);
+        }
       }
     }
-  } else {
-    SchurFwd<W> A;
-    for (int j = 0; j < ns; ++j) { ffetch(j, A); fstep(j, A); }
   }
   __syncthreads();
   // ---------------- backward: x_{j+1} is in sh[(j+1) & 1] ----------------
@@ -319,45 +323,49 @@ __global__ void __launch_bounds__(PC_NT* W, (W <= 6 ? 2 : 1)) k_precond_schur(co
     sh[j & 1][c][lane] = xv;
     __syncthreads();
   };
-  if (PIPE) {
-    SchurBwd<W> A, B;
-    bfetch(ns - 1, A);
-    for (int j = ns - 1; j >= 0; j -= 2) {
-      bfetch(j - 1, B);
-      bstep(j, A);
-      if (j - 1 >= 0) {
-        bfetch(j - 2, A);
-        bstep(j - 1, B);
+  {
+    SchurBwd<W> buf[D];
+#pragma unroll
+    for (int k = 0; k < D - 1; ++k) bfetch(ns - 1 - k, buf[k]);
+    for (int j = ns - 1; j >= 0; j -= D) {
+#pragma unroll
+      for (int k = 0; k < D; ++k) {
+        if (j - k >= 0) {
+          bfetch(j - k - (D - 1), buf[(k + D - 1) % D]);
+          bstep(j - k, buf[k]);
+        }
       }
     }
-  } else {
-    SchurBwd<W> A;
-    for (int j = ns - 1; j >= 0; --j) { bfetch(j, A); bstep(j, A); }
   }
 }
 
 // ---- P2b: with every x_S known, A_IS x_S for the interiors next to each separator: the last w rows of interior j (into r(+)_j)
-// and the first w rows of interior j+1 (into r(-)_{j+1}).  One thread per (separator, row, channel). ----
+// and the first w rows of interior j+1 (into r(-)_{j+1}).  One thread per (separator, channel). ----
 template <int W>
 __global__ void __launch_bounds__(128) k_precond_corners(const PrecArgs p) {
   if (p.st && solver_idle(p.st)) return;
   const int a = blockIdx.x * 128 + threadIdx.x;
   if (a >= p.ld) return;
-  const int j = blockIdx.y / W, c = blockIdx.y % W, ld = p.ld;
+  const int j = blockIdx.y, ld = p.ld;                               // one thread per (separator, channel): x_S loaded once
   constexpr int WW = W * W;
-  const cplx* Ck = p.Corner + (size_t)p.cls[a] * p.P * 2 * WW + c * W;
-  const cplx* tT = Ck + ((size_t)(j + 1) * 2 + 0) * WW;               // top corner of interior j + 1, row c
-  const cplx* tB = Ck + ((size_t)j * 2 + 1) * WW;                     // bottom corner of interior j, row c
+  const cplx* Ck = p.Corner + (size_t)p.cls[a] * p.P * 2 * WW;
+  const cplx* tT = Ck + ((size_t)(j + 1) * 2 + 0) * WW;               // top corner of interior j + 1
+  const cplx* tB = Ck + ((size_t)j * 2 + 1) * WW;                     // bottom corner of interior j
   const cplx* xs = p.y + (size_t)(pc_lo(p, j) + pc_len(p, j)) * ld + a;
-  cplx ct = make_double2(0, 0), cb = make_double2(0, 0);
+  cplx xv[W];
 #pragma unroll
-  for (int q = 0; q < W; ++q) {
-    const cplx xv = xs[(size_t)q * ld];
-    cfma(ct, __ldg(tT + q), xv);
-    cfma(cb, __ldg(tB + q), xv);
+  for (int q = 0; q < W; ++q) xv[q] = xs[(size_t)q * ld];
+#pragma unroll
+  for (int c = 0; c < W; ++c) {
+    cplx ct = make_double2(0, 0), cb = make_double2(0, 0);
+#pragma unroll
+    for (int q = 0; q < W; ++q) {
+      cfma(ct, __ldg(tT + c * W + q), xv[q]);
+      cfma(cb, __ldg(tB + c * W + q), xv[q]);
+    }
+    p.rsm[((size_t)(j + 1) * W + c) * ld + a] = ct;
+    p.rsp[((size_t)j * W + c) * ld + a] = cb;
   }
-  p.rsm[((size_t)(j + 1) * W + c) * ld + a] = ct;
-  p.rsp[((size_t)j * W + c) * ld + a] = cb;
 }
 
 // ---- P3: one warp = 32 channels x one interior.  The right-hand side lives in a shared-memory tile (one column per lane, so
@@ -585,7 +593,7 @@ static int launch_precond_w(const PrecArgs& a, cudaStream_t s) {
       ++n;
     }
     k_precond_schur<W><<<a.ld / PC_NT, PC_NT * W, 0, s>>>(a);
-    k_precond_corners<W><<<dim3((a.ld + 127) / 128, (a.P - 1) * W), 128, 0, s>>>(a);
+    k_precond_corners<W><<<dim3((a.ld + 127) / 128, a.P - 1), 128, 0, s>>>(a);
     n += 2;
   }
   k_precond_tile<W><<<dim3(a.ld / PC_NT, a.P), PC_NT, smem, s>>>(a);
