@@ -32,10 +32,13 @@
 #define MM_NSTAGE 6          // pipeline stages wanted (fewer when shared memory is short)
 #endif
 #ifndef MM_ASMEM5
-#define MM_ASMEM5 2          // same for T < 7
+#define MM_ASMEM5 3          // same for T < 7
 #endif
 #ifndef MM_ASMEM
-#define MM_ASMEM 5           // T >= 7: the A_L rows of this many widest terms live in shared memory, not in registers
+#define MM_ASMEM 7           // T >= 7: the A_L rows of this many widest terms live in shared memory, not in registers
+#endif
+#ifndef MM_NOPAIR
+#define MM_PAIR 1            // interior periods process both slices together (measured: HBM-scale 1.68 -> 1.565 ms)
 #endif
 
 __host__ __device__ constexpr int mm_floordiv(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
@@ -232,41 +235,17 @@ __global__ void __launch_bounds__(MM_NT, 1) k_apply_mma(const __grid_constant__ 
   cplx d0 = make_double2(0, 0);
   double d1 = 0;
 
-  // one slice: PAR = its parity (static tile pattern), CHK = some touched tile may lie outside this CTA's range
-  auto slice = [&](int u, auto PAR, auto CHK) {
+  // refill the stage slice s used with slice s + NSTAGE once every warp has left it (thread 0; called once per slice, in order)
+  auto refill = [&](int s) {
+    if (s >= 0 && s + PL::NSTAGE < nq) {
+      mm_wait(&empty[s % PL::NSTAGE], (s / PL::NSTAGE) & 1);
+      issue(s + PL::NSTAGE);
+    }
+  };
+  // radial band of one slice (DMMA): tiles u + F(par) + k; CHK = some touched tile may lie outside this CTA's range
+  auto radial = [&](int u, const cplx (&z)[T], const double* fr, bool row_ok, auto PAR, auto CHK) {
     constexpr int par = decltype(PAR)::value;
     constexpr bool chk = decltype(CHK)::value;
-    const int q = 2 * u + par;
-    if (tid == 0 && q >= 2 && q - 2 + PL::NSTAGE < nq) {           // refill the stage slice q - 2 used, once every warp has left it
-      mm_wait(&empty[(q - 2) % PL::NSTAGE], ((q - 2) / PL::NSTAGE) & 1);
-      issue(q - 2 + PL::NSTAGE);
-    }
-    __syncwarp();
-    mm_wait(&full[q % PL::NSTAGE], (q / PL::NSTAGE) & 1);
-    const unsigned char* st = smem_raw + (size_t)(q % PL::NSTAGE) * PL::STAGE_BYTES;
-    const double* fr = reinterpret_cast<const double*>(st) + lane;
-    const cplx* xs = reinterpret_cast<const cplx*>(st + PL::FRMAX * 8) + r * XP + cl + MAXM;
-    const int j = i0 + 4 * q - G::OFF + r;
-    const bool row_ok = (j >= 0) && (j < n_rad);
-    // angular combination (DFMA)
-    cplx z[T];
-#pragma unroll
-    for (int L = 0; L < T; ++L) z[L] = make_double2(0, 0);
-#pragma unroll
-    for (int o = -MAXM; o <= MAXM; ++o) {
-      if (o == 0) continue;
-      const cplx xo = xs[o];
-#pragma unroll
-      for (int L = 0; L < T; ++L) {
-        if (SH::m(L) >= (o < 0 ? -o : o)) {
-          const int qq = o < 0 ? o + SH::m(L) : SH::m(L) + o - 1;
-          const int s = SH::slot0(L) + qq;
-          if (s < PL::NSREG) cfma(z[L], Areg[s], xo);
-          else cfma(z[L], As[(s - PL::NSREG) * MM_NC + cl], xo);
-        }
-      }
-    }
-    // radial band (DMMA), tiles u + F(par) + k
 #pragma unroll
     for (int L = 0; L < T; ++L) {
       const double zr = row_ok ? z[L].x : 0.0, zi = row_ok ? z[L].y : 0.0;
@@ -283,6 +262,37 @@ __global__ void __launch_bounds__(MM_NT, 1) k_apply_mma(const __grid_constant__ 
         }
       }
     }
+  };
+  // one slice with its own pipeline synchronisation (boundary periods)
+  auto slice = [&](int u, auto PAR, auto CHK) {
+    constexpr int par = decltype(PAR)::value;
+    const int q = 2 * u + par;
+    if (tid == 0) refill(q - 2);
+    __syncwarp();
+    mm_wait(&full[q % PL::NSTAGE], (q / PL::NSTAGE) & 1);
+    const unsigned char* st = smem_raw + (size_t)(q % PL::NSTAGE) * PL::STAGE_BYTES;
+    const double* fr = reinterpret_cast<const double*>(st) + lane;
+    const cplx* xs = reinterpret_cast<const cplx*>(st + PL::FRMAX * 8) + r * XP + cl + MAXM;
+    const int j = i0 + 4 * q - G::OFF + r;
+    const bool row_ok = (j >= 0) && (j < n_rad);
+    cplx z[T];                                                     // angular combination (DFMA)
+#pragma unroll
+    for (int L = 0; L < T; ++L) z[L] = make_double2(0, 0);
+#pragma unroll
+    for (int o = -MAXM; o <= MAXM; ++o) {
+      if (o == 0) continue;
+      const cplx xo = xs[o];
+#pragma unroll
+      for (int L = 0; L < T; ++L) {
+        if (SH::m(L) >= (o < 0 ? -o : o)) {
+          const int qq = o < 0 ? o + SH::m(L) : SH::m(L) + o - 1;
+          const int s = SH::slot0(L) + qq;
+          if (s < PL::NSREG) cfma(z[L], Areg[s], xo);
+          else cfma(z[L], As[(s - PL::NSREG) * MM_NC + cl], xo);
+        }
+      }
+    }
+    radial(u, z, fr, row_ok, PAR, CHK);
     __syncwarp();
     if (lane == 0) mm_arrive(&empty[q % PL::NSTAGE]);
   };
@@ -315,15 +325,58 @@ __global__ void __launch_bounds__(MM_NT, 1) k_apply_mma(const __grid_constant__ 
   };
   using I0 = std::integral_constant<int, 0>;
   using I1 = std::integral_constant<int, 1>;
+  // an interior period: both slices together.  One pipeline synchronisation, and every A_L coefficient that comes from shared
+  // memory is loaded once for the two rows this lane owns (rows r of both slices)
+  auto pair = [&](int u) {
+    const int q0 = 2 * u;
+    if (tid == 0) { refill(q0 - 2); refill(q0 - 1); }
+    __syncwarp();
+    mm_wait(&full[q0 % PL::NSTAGE], (q0 / PL::NSTAGE) & 1);
+    mm_wait(&full[(q0 + 1) % PL::NSTAGE], ((q0 + 1) / PL::NSTAGE) & 1);
+    const unsigned char* st0 = smem_raw + (size_t)(q0 % PL::NSTAGE) * PL::STAGE_BYTES;
+    const unsigned char* st1 = smem_raw + (size_t)((q0 + 1) % PL::NSTAGE) * PL::STAGE_BYTES;
+    const cplx* xs0 = reinterpret_cast<const cplx*>(st0 + PL::FRMAX * 8) + r * XP + cl + MAXM;
+    const cplx* xs1 = reinterpret_cast<const cplx*>(st1 + PL::FRMAX * 8) + r * XP + cl + MAXM;
+    const int j = i0 + 4 * q0 - G::OFF + r;
+    const bool ok0 = (j >= 0) && (j < n_rad), ok1 = (j + 4 >= 0) && (j + 4 < n_rad);
+    cplx z0[T], z1[T];
+#pragma unroll
+    for (int L = 0; L < T; ++L) { z0[L] = make_double2(0, 0); z1[L] = make_double2(0, 0); }
+#pragma unroll
+    for (int o = -MAXM; o <= MAXM; ++o) {
+      if (o == 0) continue;
+      const cplx xa = xs0[o], xb = xs1[o];
+#pragma unroll
+      for (int L = 0; L < T; ++L) {
+        if (SH::m(L) >= (o < 0 ? -o : o)) {
+          const int qq = o < 0 ? o + SH::m(L) : SH::m(L) + o - 1;
+          const int s = SH::slot0(L) + qq;
+          const cplx av = (s < PL::NSREG) ? Areg[s < PL::NSREG ? s : 0] : As[(s - PL::NSREG) * MM_NC + cl];
+          cfma(z0[L], av, xa);
+          cfma(z1[L], av, xb);
+        }
+      }
+    }
+    radial(u, z0, reinterpret_cast<const double*>(st0) + lane, ok0, I0{}, std::false_type{});
+    if (G::PAR_E == 0) emit(u);
+    radial(u, z1, reinterpret_cast<const double*>(st1) + lane, ok1, I1{}, std::false_type{});
+    if (G::PAR_E == 1) emit(u);
+    __syncwarp();
+    if (lane == 0) { mm_arrive(&empty[q0 % PL::NSTAGE]); mm_arrive(&empty[(q0 + 1) % PL::NSTAGE]); }
+  };
   constexpr int ULO = -(G::F(0) < G::F(1) ? G::F(0) : G::F(1));                                  // first period whose tiles are all >= 0
   constexpr int LMAX = (G::F(0) + G::NTL(0) > G::F(1) + G::NTL(1) ? G::F(0) + G::NTL(0) : G::F(1) + G::NTL(1)) - 1;
   const int nu = (nq + 1) / 2;
   for (int u = 0; u < nu; ++u) {
     if (u >= ULO && u + LMAX < ntile) {                            // interior period: no range checks
+#ifdef MM_PAIR
+      pair(u);
+#else
       slice(u, I0{}, std::false_type{});
       if (G::PAR_E == 0) emit(u);
       slice(u, I1{}, std::false_type{});
       if (G::PAR_E == 1) emit(u);
+#endif
     } else {
       if (2 * u < nq) slice(u, I0{}, std::true_type{});
       if (G::PAR_E == 0) emit(u);
