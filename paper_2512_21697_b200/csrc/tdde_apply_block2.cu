@@ -1,0 +1,165 @@
+// tdde_apply_block2.cu -- start of a CN step, block parts only: ONE pass over c gives  u = oscale * H0 c  and  v = S c
+// (SURVEY 8(a) a2 + a3; R6: b = S c + r0 / 2, r0 = -i dt (H0 c + sum_L g_L (A_L (x) R_L) c)).
+// The coupling part of r0 is then added by the DMMA apply (tdde_apply_mma.cu), whose epilogue also forms ||b||^2 and ||r0||^2.
+// HBM-bound (16 B read, 32 B written, 2 (2W+1) complex FMAs per element): lane <-> channel, a thread walks a radial segment in
+// scatter form with two register windows; the x rows and the column coefficients of the CTA's kappa-classes (both operators) arrive
+// by 1-D TMA bulk copies in a three-stage mbarrier ring.
+#include "tdde_reduce.cuh"
+
+#define B2_NC TDDE_AP_NC
+#define B2_JC 4
+#define B2_NST 3
+#define B2_MAXC TDDE_AP_MAXC
+
+namespace {
+__device__ __forceinline__ uint32_t b2_smem(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void b2_bar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(b2_smem(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void b2_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(b2_smem(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void b2_bulk(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(b2_smem(dst)),
+               "l"(src), "r"(bytes), "r"(b2_smem(bar))
+               : "memory");
+}
+__device__ __forceinline__ void b2_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(ok)
+                 : "r"(b2_smem(bar)), "r"(parity)
+                 : "memory");
+  } while (!ok);
+}
+}  // namespace
+
+// stage = [blk: ncm classes x JC rows x ND][blk2: same][x: JC rows x 128]; ncm = the largest number of kappa-classes any CTA stages
+template <int W>
+struct Block2Plan {
+  static constexpr int ND = 2 * W + 1;
+  __host__ __device__ static int cs(int ncm) { return ncm * B2_JC * ND; }
+  __host__ __device__ static int stage(int ncm) { return 2 * cs(ncm) + B2_JC * B2_NC; }
+  static size_t smem(int ncm) { return (size_t)B2_NST * stage(ncm) * sizeof(cplx) + 64; }
+};
+
+// p.x -> p.y = oscale * (blk) x, p.y2 = (blk2) x; blk / blk2 in column-band form [n_cls][n_rad][2W+1]
+template <int W>
+__global__ void __launch_bounds__(B2_NC, (W <= 3 ? 4 : W <= 6 ? 3 : 2)) k_block_dual(const __grid_constant__ ApplyArgs p, const cplx* __restrict__ blk2) {
+  using PL = Block2Plan<W>;
+  constexpr int ND = PL::ND, JC = B2_JC;
+  if (p.guard == 2 && (p.red.st->stalled | (p.red.st->status != 0))) return;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  cplx* stage_base = reinterpret_cast<cplx*>(smem_raw);
+  const int CS = PL::cs(p.n_cta_cls), STAGE = PL::stage(p.n_cta_cls);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)B2_NST * STAGE * sizeof(cplx));
+
+  const int tid = threadIdx.x, ld = p.ld, n_rad = p.n_rad;
+  const int a0 = blockIdx.x * B2_NC, a = a0 + tid;
+  const bool lane_ok = a < ld;
+  const int ac = lane_ok ? a : ld - 1;
+  const int i0 = blockIdx.y * p.seg_len, i1 = min(n_rad, i0 + p.seg_len);
+  const int jlo = max(0, i0 - W), jhi = min(n_rad, i1 + W), jend = i1 + W;
+  const int nchunks = (jend - jlo + JC - 1) / JC;
+  const int slot = p.slot[ac];
+  const size_t cls_off = (size_t)p.cls[ac] * n_rad * ND;
+  const int* cta_cls = p.cta_cls + blockIdx.x * B2_MAXC;
+  const int nch = min(B2_NC, ld - a0);                        // channels of this CTA inside the vector
+  if (nch < B2_NC)
+    for (int q = tid; q < B2_NST * STAGE; q += B2_NC) stage_base[q] = make_double2(0, 0);
+  if (tid == 0) {
+    for (int q = 0; q < B2_NST; ++q) b2_bar_init(&full[q], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+
+  auto issue = [&](int c) {
+    cplx* st = stage_base + (size_t)(c % B2_NST) * STAGE;
+    uint64_t* bar = &full[c % B2_NST];
+    const int j = jlo + c * JC;
+    const int nr = min(JC, jhi - j);
+    if (nr <= 0) return;
+    int ncls = 0;
+#pragma unroll
+    for (int q = 0; q < B2_MAXC; ++q) ncls += (cta_cls[q] >= 0);
+    b2_expect_tx(bar, (uint32_t)((2 * ncls * nr * ND + nr * nch) * sizeof(cplx)));
+#pragma unroll
+    for (int q = 0; q < B2_MAXC; ++q) {
+      const int kk = cta_cls[q];
+      if (kk >= 0) {
+        b2_bulk(st + (size_t)q * JC * ND, p.blk + ((size_t)kk * n_rad + j) * ND, (uint32_t)nr * ND * sizeof(cplx), bar);
+        b2_bulk(st + CS + (size_t)q * JC * ND, blk2 + ((size_t)kk * n_rad + j) * ND, (uint32_t)nr * ND * sizeof(cplx), bar);
+      }
+    }
+    for (int r = 0; r < nr; ++r)
+      b2_bulk(st + 2 * CS + (size_t)r * B2_NC, p.x + (size_t)(j + r) * ld + a0, (uint32_t)nch * sizeof(cplx), bar);
+  };
+  if (tid == 0)
+    for (int c = 0; c < B2_NST && c < nchunks; ++c) issue(c);
+
+  cplx w1[ND], w2[ND];
+#pragma unroll
+  for (int e = 0; e < ND; ++e) { w1[e] = make_double2(0, 0); w2[e] = make_double2(0, 0); }
+  for (int c = 0; c < nchunks; ++c) {
+    const cplx* st = stage_base + (size_t)(c % B2_NST) * STAGE;
+    const int jc0 = jlo + c * JC;
+    const int nr_real = min(JC, jhi - jc0), nr_all = min(JC, jend - jc0);
+    if (nr_real > 0) b2_wait(&full[c % B2_NST], (c / B2_NST) & 1);
+#pragma unroll(W >= 6 ? 1 : 2)
+    for (int r = 0; r < JC; ++r) {
+      if (r < nr_all) {
+        if (r < nr_real) {
+          const cplx x0 = st[2 * CS + r * B2_NC + tid];
+          if (slot >= 0) {
+            const cplx* c1 = st + ((size_t)slot * JC + r) * ND;
+            const cplx* c2 = c1 + CS;
+#pragma unroll
+            for (int e = 0; e < ND; ++e) { cfma(w1[e], c1[e], x0); cfma(w2[e], c2[e], x0); }
+          } else {
+            const cplx* c1 = p.blk + cls_off + (size_t)(jc0 + r) * ND;
+            const cplx* c2 = blk2 + cls_off + (size_t)(jc0 + r) * ND;
+#pragma unroll
+            for (int e = 0; e < ND; ++e) { cfma(w1[e], __ldg(c1 + e), x0); cfma(w2[e], __ldg(c2 + e), x0); }
+          }
+        }
+        const int i = jc0 + r - W;
+        if (i >= i0 && lane_ok) {
+          p.y[(size_t)i * ld + a] = cmul(p.oscale, w1[0]);
+          p.y2[(size_t)i * ld + a] = w2[0];
+        }
+#pragma unroll
+        for (int e = 0; e < ND - 1; ++e) { w1[e] = w1[e + 1]; w2[e] = w2[e + 1]; }
+        w1[ND - 1] = make_double2(0, 0); w2[ND - 1] = make_double2(0, 0);
+      }
+    }
+    __syncthreads();                                            // everybody is done with stage c % NST
+    if (tid == 0 && c + B2_NST < nchunks) issue(c + B2_NST);
+  }
+}
+
+template <int W>
+static int launch_block_dual_w(const ApplyArgs& a, const cplx* blk2, cudaStream_t s) {
+  static bool attr_set[64] = {};
+  const size_t smem = Block2Plan<W>::smem(a.n_cta_cls);
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev < 0 || dev >= 64 || !attr_set[dev]) {
+    if (cudaFuncSetAttribute(k_block_dual<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Block2Plan<W>::smem(B2_MAXC)) != cudaSuccess) return -2;
+    if (dev >= 0 && dev < 64) attr_set[dev] = true;
+  }
+  dim3 grid((a.ld + B2_NC - 1) / B2_NC, (a.n_rad + a.seg_len - 1) / a.seg_len);
+  k_block_dual<W><<<grid, B2_NC, smem, s>>>(a, blk2);
+  return 1;
+}
+
+// y = oscale * (blk) x, y2 = (blk2) x; W = the (padded) half-bandwidth of the banded path's column bands
+int launch_block_dual(const ApplyArgs& a, const cplx* blk2, int W, cudaStream_t s) {
+  switch (W) {
+    case 3: return launch_block_dual_w<3>(a, blk2, s);
+    case 6: return launch_block_dual_w<6>(a, blk2, s);
+    case 9: return launch_block_dual_w<9>(a, blk2, s);
+    default: return -1;
+  }
+}

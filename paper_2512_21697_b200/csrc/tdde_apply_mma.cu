@@ -308,7 +308,13 @@ __global__ void __launch_bounds__(MM_NT, 1) k_apply_mma(const __grid_constant__ 
         if (i < i1 && lane_ok) {
           cplx yv = make_double2(pv[e].x + (acc[0][0][e] - acc[0][2][e]), pv[e].y + (acc[0][0][e] + acc[0][1][e]));
           p.y[(size_t)i * ld + a] = yv;
-          cfma_conj(d0, pa[e], yv);
+          if (p.emode == 3) {                                      // start of step: y = y2 = r0, aux = S c: ||S c + r0 / 2||^2, ||r0||^2
+            p.y2[(size_t)i * ld + a] = yv;
+            const double bx = fma(0.5, yv.x, pa[e].x), by = fma(0.5, yv.y, pa[e].y);
+            d0.x = fma(bx, bx, d0.x); d0.x = fma(by, by, d0.x);
+          } else {
+            cfma_conj(d0, pa[e], yv);
+          }
           d1 = fma(yv.x, yv.x, d1); d1 = fma(yv.y, yv.y, d1);
         }
       }
@@ -465,7 +471,7 @@ static int launch_mma_one(const ApplyArgs& a, dim3 grid, cudaStream_t s) {
 
 // y = addv + (coupling terms) x with fused <aux, y>, ||y||^2; a.seg_len must be a multiple of 8
 int launch_apply_mma(const ApplyArgs& a, int T, int m0, int mstep, int W, cudaStream_t s) {
-  if (!a.addv || !a.Rfrag || a.emode != 0 || (a.seg_len & 7)) return -1;
+  if (!a.addv || !a.Rfrag || (a.emode != 0 && a.emode != 3) || (a.emode == 3 && (!a.aux || !a.y2)) || (a.seg_len & 7)) return -1;
   dim3 grid((a.ld + MM_NC - 1) / MM_NC, (a.n_rad + a.seg_len - 1) / a.seg_len);
 #define X(t, aa, b, w) if (T == t && m0 == aa && mstep == b && W == w) return launch_mma_one<t, aa, b, w>(a, grid, s);
   TDDE_MMA_SHAPES(X)

@@ -387,6 +387,7 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     // (used by the banded apply and by the preconditioner's correction kernel)
     const int n_cta = (h->ld + TDDE_AP_NC - 1) / TDDE_AP_NC;
     std::vector<int> slot(h->ld, -1), cta_cls((size_t)n_cta * TDDE_AP_MAXC, -1);
+    int cmax = 0;
     for (int b = 0; b < n_cta; ++b) {
       int cnt = 0;
       for (int a = b * TDDE_AP_NC; a < std::min(h->ld, (b + 1) * TDDE_AP_NC); ++a) {
@@ -396,7 +397,9 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
         if (q == cnt && cnt < TDDE_AP_MAXC) cta_cls[(size_t)b * TDDE_AP_MAXC + cnt++] = k;
         slot[a] = q < cnt ? q : -1;
       }
+      cmax = std::max(cmax, cnt);
     }
+    h->cta_cls_max = std::max(1, cmax);
     int rc;
     if ((rc = dev_upload(&h->d_slot, slot.data(), slot.size(), s))) return rc;
     if ((rc = dev_upload(&h->d_cta_cls, cta_cls.data(), cta_cls.size(), s))) return rc;
@@ -428,6 +431,12 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
         }
         h->seg_len_m = best_seg;
         if (const char* env = std::getenv("TDDE_MMA_SEG")) h->seg_len_m = std::max(8, std::atoi(env) / 8 * 8);
+        // Start of step as block pass + DMMA coupling apply.  Measured on B200 (ms per step, split / one H-apply + S-apply): HBM-scale
+        // T = 7, W = 6: 7.85 / 8.01; W = 9: 10.74 / 10.60 (the two 19-entry windows of the block pass do not fit); Large T = 5:
+        // 1.566 / 1.554.  So: only where the register-window kernel needs its two-group term split (T >= 6) and the block pass keeps
+        // both windows in registers (W <= 6).  TDDE_SPLIT_START / TDDE_NO_SPLIT_START force it (tests).
+        h->split_start = h->use_subst && ((T >= 6 && h->bW <= 6) || std::getenv("TDDE_SPLIT_START"));
+        if (std::getenv("TDDE_NO_SPLIT_START")) h->split_start = false;
       }
     }
     if (h->path == 2) {

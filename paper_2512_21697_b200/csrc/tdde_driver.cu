@@ -50,7 +50,7 @@ int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int b
     a.Rall = h->d_Rall; a.slot = h->d_slot; a.cta_cls = h->d_cta_cls;
     a.Aoff = h->d_Aoff;
     rc = -1;
-    if (a.addv && T > 0 && emode == 0 && h->seg_len_m > 0) {      // in-iteration apply: DMMA variant
+    if (a.addv && T > 0 && (emode == 0 || emode == 3) && h->seg_len_m > 0) {      // y = addv + coupling terms: DMMA variant
       a.Rfrag = h->d_Rfrag;
       a.seg_len = h->seg_len_m;
       rc = launch_apply_mma(a, T, h->bM0, h->bMS, h->bW, h->stream);
@@ -153,6 +153,23 @@ static int enqueue_step_start(tdde_handle* h) {
   SolverState* st = h->d_st;
   const cplx one = make_double2(1.0, 0.0);
   int rc;
+  if (h->split_start) {
+    // Shapes with a DMMA apply: one HBM-bound pass gives the block parts  r = -i dt H0 c  and  s = S c,  then the DMMA apply adds the
+    // coupling part in place, r = rhat = r + (-i dt) sum_L g_L (A_L (x) R_L) c, and forms ||b||^2 = ||S c + r0 / 2||^2 and ||r0||^2
+    ApplyArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.x = h->X; a.y = h->r; a.y2 = h->s; a.oscale = make_double2(0.0, -h->cfg.dt);
+    a.n_ang = h->cfg.n_ang; a.n_rad = h->cfg.n_rad; a.ld = h->ld; a.seg_len = h->seg_len_s;
+    a.cls = h->d_cls; a.blk = h->d_H0; a.slot = h->d_slot; a.cta_cls = h->d_cta_cls; a.n_cta_cls = h->cta_cls_max;
+    a.guard = 2; a.red.st = st;
+    rc = launch_block_dual(a, h->d_S, h->bW, h->stream);
+    if (rc == -2) return tdde_cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(block_dual)");
+    if (rc > 0) {
+      h->launches += rc;
+      return enqueue_apply(h, h->X, h->r, h->s, BLK_H0, make_double2(0.0, -h->cfg.dt), true, h->d_g, &st->step_idx, 2, FIN_R0, st, h->r, 3,
+                           one, h->rhat);
+    }
+  }
   // r0 = rhat = -i dt H c and ||r0||^2, written by the H-apply itself
   if ((rc = enqueue_apply(h, h->X, h->r, nullptr, BLK_H0, one, true, h->d_g, &st->step_idx, 2, FIN_RES0, st, nullptr, 1,
                           make_double2(0.0, -h->cfg.dt), h->rhat)))

@@ -34,6 +34,7 @@ struct tdde_handle {
   int seg_len = 0;               // radial rows per thread (banded path)
   int seg_len_m = 0;             // radial rows per CTA of the DMMA apply (multiple of 8); 0 = that kernel is not used
   double* d_Rfrag = nullptr;     // its B-operand fragment table
+  bool split_start = false;      // start of step = block pass (k_block_dual) + DMMA coupling apply instead of H-apply + S-apply
   int seg_len_s = 0;             // radial rows per thread for the S-only (T = 0) apply: latency-bound, wants more CTAs
   int apply_ng = 1;              // warp groups the terms are split over (banded path)
   bool norm_banded = false;      // S-only apply can use the banded T=0 kernel
@@ -47,6 +48,7 @@ struct tdde_handle {
   cplx* d_Aoff = nullptr;                    // banded path
   cplx* d_Rall = nullptr;                    // banded path: [n_rad][T][2w+1]
   int *d_slot = nullptr, *d_cta_cls = nullptr;
+  int cta_cls_max = TDDE_AP_MAXC;            // largest number of classes staged by one 128-channel CTA
   int* d_Arowptr[TDDE_MAX_TERMS] = {};       // generic path
   int* d_Acol[TDDE_MAX_TERMS] = {};
   cplx* d_Aval[TDDE_MAX_TERMS] = {};

@@ -97,7 +97,8 @@ struct ApplyArgs {
   const cplx* x;           // internal layout
   cplx* y;
   const cplx* aux;         // vector for the fused dot (nullable)
-  int emode;               // write-out: 0 y = result; 1 y = y2 = oscale * result (r0 and rhat); 2 nothing stored,
+  int emode;               // write-out: 0 y = result; 1 y = y2 = oscale * result (r0 and rhat); 3 (k_apply_mma) y = y2 = result,
+                           //   d0.x accumulates |aux + result / 2|^2 (||b||^2 with aux = S c), d1 = ||result||^2; 2 nothing stored,
                            //   d1 accumulates |result + aux / 2|^2 (||b||^2 with aux = r0, R6)
   cplx oscale;
   cplx* y2;
@@ -113,6 +114,7 @@ struct ApplyArgs {
   const cplx* Rall;        // banded path: column-band of every term interleaved [n_rad][T][2w+1]: Rall[j][L][e] = R_L[j-w+e][j]
   const int* slot;         // [ld] index of the channel's class in its CTA's class list, -1 = not staged
   const int* cta_cls;      // [n_cta][TDDE_AP_MAXC] classes staged per CTA (-1 = unused)
+  int n_cta_cls;           // k_block_dual: the largest number of classes any CTA stages (sizes its shared-memory stage)
   const cplx* Aoff;        // banded path: [n_slots][ld], slot = (term, offset) in kernel order
   const double* Rfrag;     // DMMA path (tdde_apply_mma.cu): B-operand fragments of every 4-row slice, nullable
   // staged sparse-A path (tdde_apply_sparse.cu): ELL rows of every term, slot-major [sp_nslots][ld]; blk and Rall padded to 2W+1
@@ -184,6 +186,7 @@ bool apply_mma_available(int T, int m0, int mstep, int W);
 int apply_mma_halo(int W);
 int apply_mma_channels();
 int launch_apply_mma(const ApplyArgs& a, int T, int m0, int mstep, int W, cudaStream_t s);
+int launch_block_dual(const ApplyArgs& a, const cplx* blk2, int W, cudaStream_t s);   // y = oscale (blk) x, y2 = (blk2) x
 int launch_apply_sparse(const ApplyArgs& a, int W, cudaStream_t s);
 size_t apply_sparse_smem(int W, int T, int nslots, int xw, bool a_in_smem);
 int launch_precond(const PrecArgs& a, cudaStream_t s);

@@ -860,3 +860,27 @@ def test_mma_and_window_propagation_agree(monkeypatch):
     assert rel(out[0][0], out[1][0]) <= 1e-13
     assert rel(out[0][0], c_ref) <= 1e-9 and rel(out[1][0], c_ref) <= 1e-9
     assert abs(out[0][1] - sum(i.half_iters for i in infos)) <= 4
+
+
+@pytest.mark.parametrize("bw,T", [(13, 7), (19, 7), (13, 5), (7, 7)])
+def test_split_start_of_step_matches_single_apply_start(bw, T, monkeypatch):
+    """Start of a step as block pass (r = -i dt H0 c, s = S c) + DMMA coupling apply with the ||b||^2 / ||r0||^2 epilogue
+    (TDDE_SPLIT_START forces it for every shape that has a DMMA kernel) against the single H-apply + S-apply start: same iteration
+    counts, states equal to rounding, both within 1e-9 of the oracle; radial size not a multiple of 8, ragged channel count."""
+    from paper_2512_21697_b200 import Tdde
+    p = tdde_inputs.make_synthetic(n_ang=230, n_r=43, bandwidth=bw, n_terms=T, dt=0.01, n_steps=3, rtol=1e-10, seed=5 + bw, name="split",
+                                   phase=np.pi / 2, e0=1.5)
+    ops, fact = orc.assemble(p), orc.factor_precond(p)
+    c_ref, infos = orc.propagate(p, ops, fact, p.c0, 3)
+    out = []
+    for env in ("TDDE_SPLIT_START", "TDDE_NO_SPLIT_START"):
+        monkeypatch.delenv("TDDE_SPLIT_START", raising=False)
+        monkeypatch.setenv(env, "1")
+        prop = Tdde(p)
+        c = prop.to_device(p.c0)
+        st = prop.propagate(c, p.g_table(3))
+        out.append((c.cpu().numpy(), st["half_iters"], st["rel_res"]))
+        prop.close()
+    assert out[0][1] == out[1][1]
+    assert rel(out[0][0], out[1][0]) <= 1e-13
+    assert rel(out[0][0], c_ref) <= 1e-9 and rel(out[1][0], c_ref) <= 1e-9
