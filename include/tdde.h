@@ -134,6 +134,37 @@ int tdde_project(tdde_handle* h, const tdde_c64* c_dev, double* P_host);
 int tdde_eigensolve(int32_t n_cls, int32_t n_rad, int32_t w0, const tdde_c64* S_band, const tdde_c64* H0_band, double* E_host,
                     tdde_c64* V_host, void* cuda_stream);
 
+/* ---- Channel-slab sharding over several GPUs (SURVEY 8(f) NEXT-3; PAPER.md:279-297 section 3.2, :307 section 3.3) ----
+ * The paper partitions the angular channels among the ranks, exchanges the coupled x-slabs before every operator apply, keeps the
+ * block-diagonal preconditioner rank-local and sums every inner product over the ranks.  Here: a SHARD is an ordinary handle created
+ * from the rank-local problem (channels [halo | owned | halo] renumbered from 0, rows of every A_L for the owned channels only;
+ * paper_2512_21697_b200/sharding.py builds it), a GROUP drives the shards of one process in lock step:
+ *   before each apply the halo channels of its input vector are refreshed from their owners (device copies between local shards,
+ *   pack + ncclSend/ncclRecv + unpack between ranks); every kernel writes and sums owned channels only; the three partial sums of a
+ *   fused reduction are all-reduced (ncclAllReduce) between the kernel's block pass and the scalar update (k_finalize), everything
+ *   stream-ordered; one host read of the solver state per CN step.
+ * n_local = 1 with an NCCL id = one shard per process / GPU (production); n_local = world with nccl_id = NULL = every shard in this
+ * process on one stream (how the exchange, the ownership masks and the split reductions are tested on a one-GPU box).
+ *   own_lo, own_hi : owned channels [own_lo, own_hi) in the shard's LOCAL numbering
+ *   recv_*         : halo pieces: channels [recv_lo, recv_lo + recv_n) of this shard = channels [recv_src_lo, ...) of shard recv_rank
+ *   send_*         : the same pieces seen from the owner (needed with NCCL only): channels [send_lo, send_lo + send_n) go to send_rank
+ * All shards must share n_rad, n_terms, dt, rtol, max_iter.  Errors: TDDE_EINVAL, TDDE_ENOMEM, TDDE_ECUDA (also: NCCL not loadable). */
+typedef struct tdde_group tdde_group;
+typedef struct {
+  int32_t rank, world;
+  int32_t own_lo, own_hi;
+  int32_t n_recv;
+  const int32_t *recv_rank, *recv_lo, *recv_src_lo, *recv_n;   /* host [n_recv] */
+  int32_t n_send;
+  const int32_t *send_rank, *send_lo, *send_n;                 /* host [n_send] */
+} tdde_shard;
+int  tdde_nccl_unique_id(void* id128);                          /* host, 128 bytes: rank 0 calls it, the launcher broadcasts it */
+int  tdde_group_create(tdde_group** out, int32_t n_local, tdde_handle* const* handles, const tdde_shard* shards, const void* nccl_id128);
+/* n_steps CN steps on every local shard: c_dev[k] = device state of shard k in ITS local numbering (halo entries are refreshed, owned
+ * entries advanced).  g_table as for tdde_propagate.  st (nullable): the job-wide statistics (identical on every rank).  Synchronises. */
+int  tdde_group_propagate(tdde_group* g, tdde_c64* const* c_dev, int64_t n_steps, const double* g_table, tdde_stats* st);
+void tdde_group_destroy(tdde_group* g);                         /* the handles stay alive and become ordinary handles again */
+
 /* Which operator-apply kernel the handle uses: 1 = banded A_L held in registers, 2 = general sparse A_L staged in shared memory
  * (x tile by TMA), 0 = unstaged generic CSR fall-back. */
 int tdde_apply_path(const tdde_handle* h);

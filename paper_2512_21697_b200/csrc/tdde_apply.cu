@@ -302,8 +302,8 @@ __global__ void __launch_bounds__(NG * AP_NC, (NG == 2 ? TDDE_AP_MINB2 : AP_MINB
   const int a0 = blockIdx.x * AP_NC;
   k.a = a0 + k.tid;                                          // channel; lanes with a >= ld idle along
   k.ld = p.ld; k.n_rad = p.n_rad;
-  k.lane_ok = k.a < k.ld;
-  k.ac = k.lane_ok ? k.a : k.ld - 1;
+  k.lane_ok = k.a >= p.own_lo && k.a < p.own_hi;              // own_hi <= ld
+  k.ac = k.a < k.ld ? k.a : k.ld - 1;
   k.i0 = blockIdx.y * p.seg_len;
   k.i1 = min(k.n_rad, k.i0 + p.seg_len);
   k.jlo = max(0, k.i0 - W);
@@ -391,7 +391,7 @@ __global__ void __launch_bounds__(AP_NT) k_apply_generic(const ApplyArgs p) {
   for (long long wk = blockIdx.x; wk < nwork; wk += gridDim.x) {
     const int a = (int)(wk % cb) * AP_NT + threadIdx.x;
     const int i = (int)(wk / cb);
-    if (a >= ld) continue;
+    if (a >= p.own_hi || a < p.own_lo) continue;
     cplx acc = make_double2(0, 0);
     if (a < p.n_ang) {
       const int w0 = p.w0, nd0 = 2 * w0 + 1;

@@ -153,8 +153,8 @@ __global__ void __launch_bounds__(MM_NT, 1) k_apply_mma(const __grid_constant__ 
   const int ld = p.ld, n_rad = p.n_rad;
   const int a0 = blockIdx.x * MM_NC;
   const int a = a0 + cl;
-  const bool lane_ok = a < ld;
-  const int ac = lane_ok ? a : ld - 1;
+  const bool lane_ok = a >= p.own_lo && a < p.own_hi;          // own_hi <= ld
+  const int ac = a < ld ? a : ld - 1;
   const int i0 = blockIdx.y * p.seg_len;                       // seg_len is a multiple of 8
   const int i1 = min(n_rad, i0 + p.seg_len);
   const int ntile = (i1 - i0 + 7) / 8;                         // output tiles of this CTA

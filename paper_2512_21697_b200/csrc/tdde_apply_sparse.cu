@@ -71,8 +71,8 @@ __global__ void __launch_bounds__(SP_NC, 1) k_apply_sparse(const __grid_constant
 
   const int tid = threadIdx.x, ld = p.ld, n_rad = p.n_rad;
   const int a0 = blockIdx.x * SP_NC, a = a0 + tid;
-  const bool lane_ok = a < ld;
-  const int ac = lane_ok ? a : ld - 1;
+  const bool lane_ok = a >= p.own_lo && a < p.own_hi;          // own_hi <= ld
+  const int ac = a < ld ? a : ld - 1;
   const int i0 = blockIdx.y * p.seg_len, i1 = min(n_rad, i0 + p.seg_len);
   const int jlo = max(0, i0 - W), jhi = min(n_rad, i1 + W), jend = i1 + W;
   const int nchunks = (jend - jlo + JC - 1) / JC;

@@ -36,6 +36,8 @@ int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int b
   a.w0 = h->cfg.w0;
   a.guard = guard;
   a.red.partials = h->d_partials; a.red.ticket = h->d_ticket; a.red.st = st; a.red.fin = fin;
+  a.red.shard_out = (h->shard_sums && fin != FIN_NONE) ? h->shard_sums : nullptr;
+  a.own_lo = h->own_lo; a.own_hi = h->own_hi > 0 ? h->own_hi : h->ld;
   const int T = with_terms ? h->cfg.n_terms : 0;
   a.n_terms = T;
   if (T == 0 && h->have_xmaps) {
@@ -137,6 +139,7 @@ VecArgs make_vec_args(tdde_handle* h, SolverState* st, int fin) {
   a.u = h->t;
   a.dt = h->cfg.dt;
   a.red.partials = h->d_partials; a.red.ticket = h->d_ticket; a.red.st = st; a.red.fin = fin;
+  a.red.shard_out = (h->shard_sums && fin != FIN_NONE) ? h->shard_sums : nullptr;
   return a;
 }
 
@@ -162,6 +165,7 @@ static int enqueue_step_start(tdde_handle* h) {
     a.n_ang = h->cfg.n_ang; a.n_rad = h->cfg.n_rad; a.ld = h->ld; a.seg_len = h->seg_len_s;
     a.cls = h->d_cls; a.blk = h->d_H0; a.slot = h->d_slot; a.cta_cls = h->d_cta_cls; a.n_cta_cls = h->cta_cls_max;
     a.guard = 2; a.red.st = st;
+    a.own_lo = h->own_lo; a.own_hi = h->own_hi > 0 ? h->own_hi : h->ld;
     rc = launch_block_dual(a, h->d_S, h->bW, h->stream);
     if (rc == -2) return tdde_cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(block_dual)");
     if (rc > 0) {

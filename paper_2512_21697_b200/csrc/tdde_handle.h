@@ -71,6 +71,11 @@ struct tdde_handle {
   double* d_proj = nullptr;
   int n_states = 0;
 
+  // channel-slab sharding (tdde_shard.cu): a handle that is one shard of a group owns the local channels
+  // [own_lo, own_hi) (the rest are halo inputs) and hands its reduction sums to the group instead of finalising them
+  int own_lo = 0, own_hi = 0;                // own_hi == 0: not sharded (all of [0, ld))
+  double* shard_sums = nullptr;              // device [4]
+
   // solver state, scratch
   SolverState* d_st = nullptr;
   SolverState* d_st_bench = nullptr;         // never-idle dummy state for tdde_time_kernel

@@ -88,6 +88,8 @@ struct ReduceCtx {
   unsigned int* ticket;    // zero between kernels
   SolverState* st;
   int fin;
+  double* shard_out;       // channel-slab sharding (tdde_shard.cu): the last block writes its three sums here and does NOT finalise;
+                           //   the sums are all-reduced over the ranks and k_finalize applies them.  nullptr = single GPU
 };
 
 // ---- operator apply ----
@@ -134,6 +136,7 @@ struct ApplyArgs {
   const cplx* blk_row;     // row-band block coefficients [n_cls][n_rad][2w0+1]
   int w[TDDE_MAX_TERMS];
   int w0;
+  int own_lo, own_hi;      // channels [own_lo, own_hi) are written and enter the fused sums (sharding: the owned slab; else 0, ld)
   int guard;               // 0 none; 1: no-op when st->done|stalled|status (iterations); 2: no-op when stalled|status (start of step)
   ReduceCtx red;
 };

@@ -167,7 +167,8 @@ __device__ __forceinline__ void grid_reduce_finalize(double v0, double v1, doubl
   if (threadIdx.x == 0) {
     a = b = c = 0;
     for (int k = 0; k < NT / 32; ++k) { a += sm[0][k]; b += sm[1][k]; c += sm[2][k]; }
-    finalize_scalars(rc.st, rc.fin, a, b, c);
+    if (rc.shard_out) { rc.shard_out[0] = a; rc.shard_out[1] = b; rc.shard_out[2] = c; }
+    else finalize_scalars(rc.st, rc.fin, a, b, c);
     *rc.ticket = 0u;
     __threadfence();
   }
