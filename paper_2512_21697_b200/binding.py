@@ -19,7 +19,7 @@ LIB_PATH = os.environ.get("TDDE_LIB_PATH", os.path.join(_HERE, "libtdde.so"))
 EXPORTS = [
     "tdde_create", "tdde_step", "tdde_propagate", "tdde_norm", "tdde_apply", "tdde_precond",
     "tdde_propagate_host", "tdde_step_forced", "tdde_apply_coupling", "tdde_time_kernel", "tdde_fp64_peak", "tdde_launch_count",
-    "tdde_apply_path", "tdde_iter_apply_kernel", "tdde_set_eigenstates", "tdde_project", "tdde_eigensolve", "tdde_selftest_partition", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
+    "tdde_apply_path", "tdde_iter_apply_kernel", "tdde_nccl_unique_id", "tdde_group_create", "tdde_group_propagate", "tdde_group_destroy", "tdde_set_eigenstates", "tdde_project", "tdde_eigensolve", "tdde_selftest_partition", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
 ]
 
 STATUS = {0: "TDDE_OK", -1: "TDDE_EINVAL", -2: "TDDE_ENOMEM", -3: "TDDE_ECUDA", -4: "TDDE_ESINGULAR",
@@ -46,6 +46,12 @@ class tdde_stats(C.Structure):
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+class tdde_shard(C.Structure):
+    _fields_ = [("rank", C.c_int32), ("world", C.c_int32), ("own_lo", C.c_int32), ("own_hi", C.c_int32),
+                ("n_recv", C.c_int32), ("recv_rank", C.c_void_p), ("recv_lo", C.c_void_p), ("recv_src_lo", C.c_void_p), ("recv_n", C.c_void_p),
+                ("n_send", C.c_int32), ("send_rank", C.c_void_p), ("send_lo", C.c_void_p), ("send_n", C.c_void_p)]
 
 
 class TddeError(RuntimeError):
@@ -95,6 +101,14 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.tdde_selftest_partition.restype = C.c_int
     lib.tdde_paper_variant.argtypes = [vp, vp, vp, vp, i32, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i64)]
     lib.tdde_paper_variant.restype = C.c_int
+    lib.tdde_nccl_unique_id.argtypes = [vp]
+    lib.tdde_nccl_unique_id.restype = C.c_int
+    lib.tdde_group_create.argtypes = [C.POINTER(vp), i32, vp, vp, vp]
+    lib.tdde_group_create.restype = C.c_int
+    lib.tdde_group_propagate.argtypes = [vp, vp, i64, vp, C.POINTER(tdde_stats)]
+    lib.tdde_group_propagate.restype = C.c_int
+    lib.tdde_group_destroy.argtypes = [vp]
+    lib.tdde_group_destroy.restype = None
     lib.tdde_destroy.argtypes = [vp]
     lib.tdde_destroy.restype = None
     lib.tdde_strerror.argtypes = [C.c_int]
@@ -312,6 +326,62 @@ class Tdde:
         if getattr(self, "h", None):
             self.lib.tdde_destroy(self.h)
             self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def nccl_unique_id() -> bytes:
+    """128-byte NCCL id (tdde_nccl_unique_id): rank 0 creates it, the launcher broadcasts it to the other ranks."""
+    lib = load_library()
+    buf = C.create_string_buffer(128)
+    _check(lib, lib.tdde_nccl_unique_id(buf), "tdde_nccl_unique_id")
+    return buf.raw
+
+
+class TddeGroup:
+    """The shards of one process driven in lock step (tdde_group_*).  `shards`: Tdde handles built from the
+    rank-local problems; `specs`: one dict per shard with rank, world, own_lo, own_hi and the integer lists recv_rank, recv_lo,
+    recv_src_lo, recv_n, send_rank, send_lo, send_n (paper_2512_21697_b200.sharding.shard_specs); `nccl_id`: 128 bytes for one shard
+    per process over NCCL, None when every shard of the job is in this process."""
+
+    def __init__(self, shards, specs, nccl_id: Optional[bytes] = None):
+        self.lib = load_library()
+        self.shards = list(shards)
+        self._keep = []
+        arr = (tdde_shard * len(specs))()
+
+        def ptr(v):
+            a = np.ascontiguousarray(v, dtype=np.int32)
+            self._keep.append(a)
+            return a.ctypes.data if a.size else None
+        for k, sp in enumerate(specs):
+            arr[k].rank, arr[k].world, arr[k].own_lo, arr[k].own_hi = sp["rank"], sp["world"], sp["own_lo"], sp["own_hi"]
+            arr[k].n_recv, arr[k].n_send = len(sp["recv_n"]), len(sp["send_n"])
+            arr[k].recv_rank, arr[k].recv_lo, arr[k].recv_src_lo, arr[k].recv_n = (ptr(sp[q]) for q in ("recv_rank", "recv_lo", "recv_src_lo", "recv_n"))
+            arr[k].send_rank, arr[k].send_lo, arr[k].send_n = (ptr(sp[q]) for q in ("send_rank", "send_lo", "send_n"))
+        hs = (C.c_void_p * len(self.shards))(*[sh.h for sh in self.shards])
+        self.g = C.c_void_p()
+        idbuf = C.create_string_buffer(nccl_id, 128) if nccl_id is not None else None
+        _check(self.lib, self.lib.tdde_group_create(C.byref(self.g), len(self.shards), hs, arr, idbuf), "tdde_group_create")
+
+    def propagate(self, c_devs, g_table, n_steps: Optional[int] = None):
+        g = np.asarray(g_table, dtype=np.float64)
+        n_steps = (g.shape[0] if g.ndim == 2 else 1) if n_steps is None else n_steps
+        g = _g_array(g, self.shards[0].n_terms, n_steps)
+        ptrs = (C.c_void_p * len(self.shards))(*[sh._vec(c).value for sh, c in zip(self.shards, c_devs)])
+        st = tdde_stats()
+        rc = self.lib.tdde_group_propagate(self.g, ptrs, n_steps, _np_ptr(g), C.byref(st))
+        _check(self.lib, rc, "tdde_group_propagate")
+        return st.as_dict()
+
+    def close(self):
+        if getattr(self, "g", None):
+            self.lib.tdde_group_destroy(self.g)
+            self.g = None
 
     def __del__(self):
         try:

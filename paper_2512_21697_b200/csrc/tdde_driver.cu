@@ -203,7 +203,7 @@ static int enqueue_iteration(tdde_handle* h) {
   return 0;
 }
 
-static int upload_g(tdde_handle* h, const double* g_table, long long n_steps) {
+int upload_g(tdde_handle* h, const double* g_table, long long n_steps) {
   const int T = h->cfg.n_terms;
   const long long n_req = n_steps;
   if (T == 0) { if (!h->d_g) { CU(cudaMalloc((void**)&h->d_g, sizeof(double))); h->g_cap = 1; } return 0; }
@@ -218,7 +218,7 @@ static int upload_g(tdde_handle* h, const double* g_table, long long n_steps) {
   return 0;
 }
 
-static void fill_stats(const tdde_handle* h, tdde_stats* st) {
+void fill_stats(const tdde_handle* h, tdde_stats* st) {
   if (!st) return;
   const SolverState* s = h->h_st;
   st->steps = s->steps_done; st->half_iters = s->total_half; st->applies = s->applies; st->preconds = s->preconds;

@@ -135,6 +135,8 @@ int enqueue_precond(tdde_handle* h, const cplx* x, cplx* y, const SolverState* s
 int enqueue_vec_update(tdde_handle* h, int mode, SolverState* st, bool* fused);   // mode 0: p-update, 1: s-update (+ spike products when fused)
 VecArgs make_vec_args(tdde_handle* h, SolverState* st, int fin);
 int sync_state(tdde_handle* h);
+int upload_g(tdde_handle* h, const double* g_table, long long n_steps);   // g table -> device (grows d_g)
+void fill_stats(const tdde_handle* h, tdde_stats* st);                      // from the pinned mirror of the solver state
 // g as the caller gives it ([rows][user_terms]) -> as the kernels index it ([rows][cfg.n_terms]); returns g itself when they coincide
 bool build_mma_frags(int T, int W, int n_rad, const void* Rall, std::vector<double>& out);   // tdde_apply_mma.cu
 const double* map_g(const tdde_handle* h, const double* g, long long rows, std::vector<double>& buf);

@@ -1,14 +1,14 @@
-"""Channel-slab sharding plan (SURVEY.md 8(f) NEXT-3; PAPER.md:279-297 section 3.2, :307 section 3.3) -- HOST LOGIC ONLY.
+"""Channel-slab sharding plan (SURVEY.md 8(f) NEXT-3; PAPER.md:279-297 section 3.2, :307 section 3.3) -- the host side.
 
 The paper partitions the rows (angular channels) of the coupling matrix among ranks, exchanges the x-slabs of coupled channels
 before every operator apply, keeps the block-diagonal preconditioner rank-local and sums every inner product over the ranks.
 On NVSwitch the same decomposition is: contiguous channel slabs, halo slabs of +-(coupling reach) channels gathered before each
-apply, one fused all-reduce of <= 5 scalars per half-iteration.  This module holds the index arithmetic of that decomposition --
+apply, one all-reduce of 3 partial sums per fused reduction.  This module holds the index arithmetic of that decomposition --
 which channels a rank owns, which it must receive, and the rank-local problem (owned rows of every A_L with columns renumbered
-into [halo | owned | halo]) that a per-rank `Tdde` handle would be created from.  It moves no data and computes nothing on
-vectors; the device path (halo gather fused with the apply over NVLink peer memory, scalar all-reduce between the reduction and
-the scalar update) is not built -- north_star fixes one GPU -- and `tests/test_sharding_gloo.py` exercises this plan with two
-gloo ranks on CPU against the unsharded oracle.
+into [halo | owned | halo]) that a per-rank `Tdde` handle is created from, and the exchange lists `TddeGroup` (tdde_group_* in
+include/tdde.h, csrc/tdde_shard.cu) takes.  It moves no data and computes nothing on vectors.  `tests/test_sharding_gloo.py`
+exercises the plan with two gloo ranks on CPU against the unsharded oracle; the device path is tested on one GPU with all shards
+in one process (tests/test_gpu_sharding.py).
 """
 from __future__ import annotations
 
@@ -101,3 +101,30 @@ def local_problem(problem, plan: SlabPlan):
     c0 = problem.c0.reshape(problem.n_ang, problem.n_rad)[plan.halo_lo:plan.halo_hi].reshape(-1).copy() if problem.c0.size else problem.c0
     return replace(problem, name=f"{problem.name}-rank{plan.rank}", n_ang=n_loc, cls_of_chan=problem.cls_of_chan[plan.halo_lo:plan.halo_hi].copy(),
                    terms=terms, c0=c0)
+
+
+def shard_specs(problem, world: int):
+    """[(plan, local problem, spec)] per rank; spec = the exchange lists of tdde_shard in LOCAL channel numbering:
+    recv: halo piece [recv_lo, recv_lo + n) of this rank = channels [recv_src_lo, ...) of rank recv_rank (local numbering there);
+    send: owned piece [send_lo, send_lo + n) of this rank goes to rank send_rank."""
+    plans = plan_slabs(problem, world)
+    bounds = slab_bounds(problem.n_ang, world)
+    out = []
+    for pl in plans:
+        spec = {"rank": pl.rank, "world": world, "own_lo": pl.lo - pl.halo_lo, "own_hi": pl.hi - pl.halo_lo,
+                "recv_rank": [], "recv_lo": [], "recv_src_lo": [], "recv_n": [], "send_rank": [], "send_lo": [], "send_n": []}
+        for owner, a, b in pl.needs_from(bounds):
+            spec["recv_rank"].append(owner)
+            spec["recv_lo"].append(a - pl.halo_lo)
+            spec["recv_src_lo"].append(a - plans[owner].halo_lo)
+            spec["recv_n"].append(b - a)
+        for other in plans:
+            if other.rank == pl.rank:
+                continue
+            for owner, a, b in other.needs_from(bounds):
+                if owner == pl.rank:
+                    spec["send_rank"].append(other.rank)
+                    spec["send_lo"].append(a - pl.halo_lo)
+                    spec["send_n"].append(b - a)
+        out.append((pl, local_problem(problem, pl), spec))
+    return out

@@ -155,3 +155,30 @@ def test_sharded_cn_step_equals_unsharded_oracle_gloo_world2():
     for rank, lo, hi, slab in res:
         C[lo:hi] = slab.reshape(hi - lo, p.n_rad)
     assert np.linalg.norm(C.reshape(-1) - c_ref) <= 1e-10 * np.linalg.norm(c_ref)
+
+
+def test_shard_specs_are_symmetric_and_cover_the_halos():
+    """The exchange lists handed to tdde_group_create: every halo channel of every rank is received exactly once from its owner's
+    owned slab, and each receive has the matching send on the owner (NCCL pairs them by peer)."""
+    import tdde_inputs
+    from paper_2512_21697_b200 import sharding
+    for n_ang, T, world in [(23, 3, 2), (64, 7, 4), (150, 7, 3), (40, 5, 1)]:
+        p = tdde_inputs.make_synthetic(name="spec", n_ang=n_ang, n_r=6, bandwidth=7, n_terms=T, dt=0.01, n_steps=1, rtol=1e-10, seed=1,
+                                       with_c0=False)
+        parts = sharding.shard_specs(p, world)
+        for plan, pl, sp in parts:
+            assert pl.n_ang == plan.n_local and sp["own_hi"] - sp["own_lo"] == plan.hi - plan.lo
+            covered = np.zeros(plan.n_local, dtype=int)
+            covered[sp["own_lo"]:sp["own_hi"]] += 1
+            for r, lo, src_lo, n in zip(sp["recv_rank"], sp["recv_lo"], sp["recv_src_lo"], sp["recv_n"]):
+                covered[lo:lo + n] += 1
+                oplan, _, osp = parts[r]
+                assert osp["own_lo"] <= src_lo and src_lo + n <= osp["own_hi"]                 # inside the owner's owned slab
+                assert lo + plan.halo_lo == src_lo + oplan.halo_lo                             # the same global channels
+                assert (plan.rank, src_lo, n) in list(zip(osp["send_rank"], osp["send_lo"], osp["send_n"]))
+            assert np.all(covered == 1)
+            # owned rows keep all their couplings, halo rows have none
+            for t_loc, t in zip(pl.terms, p.terms):
+                cnt = np.diff(t_loc.A_rowptr)
+                assert np.all(cnt[:sp["own_lo"]] == 0) and np.all(cnt[sp["own_hi"]:] == 0)
+                assert np.array_equal(cnt[sp["own_lo"]:sp["own_hi"]], np.diff(t.A_rowptr)[plan.lo:plan.hi])
