@@ -8,8 +8,13 @@
 
 #define B2_NC TDDE_AP_NC
 #define B2_JC 4
-#define B2_NST 3
+#ifndef B2_NST
+#define B2_NST 3      // measured: 4 stages lose (HBM-scale step 7.87 -> 8.36 ms)
+#endif
 #define B2_MAXC TDDE_AP_MAXC
+#ifndef B2_MINB6
+#define B2_MINB6 3
+#endif
 
 namespace {
 __device__ __forceinline__ uint32_t b2_smem(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -46,7 +51,7 @@ struct Block2Plan {
 
 // p.x -> p.y = oscale * (blk) x, p.y2 = (blk2) x; blk / blk2 in column-band form [n_cls][n_rad][2W+1]
 template <int W>
-__global__ void __launch_bounds__(B2_NC, (W <= 3 ? 4 : W <= 6 ? 3 : 2)) k_block_dual(const __grid_constant__ ApplyArgs p, const cplx* __restrict__ blk2) {
+__global__ void __launch_bounds__(B2_NC, (W <= 3 ? 4 : W <= 6 ? B2_MINB6 : 2)) k_block_dual(const __grid_constant__ ApplyArgs p, const cplx* __restrict__ blk2) {
   using PL = Block2Plan<W>;
   constexpr int ND = PL::ND, JC = B2_JC;
   if (p.guard == 2 && (p.red.st->stalled | (p.red.st->status != 0))) return;
@@ -84,7 +89,8 @@ __global__ void __launch_bounds__(B2_NC, (W <= 3 ? 4 : W <= 6 ? 3 : 2)) k_block_
     int ncls = 0;
 #pragma unroll
     for (int q = 0; q < B2_MAXC; ++q) ncls += (cta_cls[q] >= 0);
-    b2_expect_tx(bar, (uint32_t)((2 * ncls * nr * ND + nr * nch) * sizeof(cplx)));
+    const bool x2d = p.use_xmap != 0;                           // one tensor copy for the x rows: full box, out-of-bounds zero-filled
+    b2_expect_tx(bar, (uint32_t)((2 * ncls * nr * ND + (x2d ? JC * B2_NC : nr * nch)) * sizeof(cplx)));
 #pragma unroll
     for (int q = 0; q < B2_MAXC; ++q) {
       const int kk = cta_cls[q];
@@ -93,8 +99,15 @@ __global__ void __launch_bounds__(B2_NC, (W <= 3 ? 4 : W <= 6 ? 3 : 2)) k_block_
         b2_bulk(st + CS + (size_t)q * JC * ND, blk2 + ((size_t)kk * n_rad + j) * ND, (uint32_t)nr * ND * sizeof(cplx), bar);
       }
     }
-    for (int r = 0; r < nr; ++r)
-      b2_bulk(st + 2 * CS + (size_t)r * B2_NC, p.x + (size_t)(j + r) * ld + a0, (uint32_t)nch * sizeof(cplx), bar);
+    if (x2d) {
+      asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(
+                       b2_smem(st + 2 * CS)),
+                   "l"(reinterpret_cast<uint64_t>(&p.xmap)), "r"(2 * a0), "r"(j), "r"(b2_smem(bar))
+                   : "memory");
+    } else {
+      for (int r = 0; r < nr; ++r)
+        b2_bulk(st + 2 * CS + (size_t)r * B2_NC, p.x + (size_t)(j + r) * ld + a0, (uint32_t)nch * sizeof(cplx), bar);
+    }
   };
   if (tid == 0)
     for (int c = 0; c < B2_NST && c < nchunks; ++c) issue(c);

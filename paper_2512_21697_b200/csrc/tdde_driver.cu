@@ -166,6 +166,7 @@ static int enqueue_step_start(tdde_handle* h) {
     a.cls = h->d_cls; a.blk = h->d_H0; a.slot = h->d_slot; a.cta_cls = h->d_cta_cls; a.n_cta_cls = h->cta_cls_max;
     a.guard = 2; a.red.st = st;
     a.own_lo = h->own_lo; a.own_hi = h->own_hi > 0 ? h->own_hi : h->ld;
+    if (h->have_xmaps) { a.xmap = h->xmaps[0]; a.use_xmap = 1; }      // X is work vector 0
     rc = launch_block_dual(a, h->d_S, h->bW, h->stream);
     if (rc == -2) return tdde_cuda_fail(cudaGetLastError(), "cudaFuncSetAttribute(block_dual)");
     if (rc > 0) {
