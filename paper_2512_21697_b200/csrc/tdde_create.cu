@@ -245,9 +245,13 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
     const int slots = h->num_sms * per_sm;
     long long best_cost = -1;
     int best_seg = n_rad;
+    // a segment may be shorter than its 2 W halo rows: on a problem that cannot fill the SMs otherwise, recomputing halo rows on idle
+    // SMs is cheaper than leaving them idle (the cost below still counts the halo, so large problems keep long segments)
+    int min_seg = 4;
+    if (const char* env = std::getenv("TDDE_MIN_SEG")) min_seg = std::max(1, std::atoi(env));
     for (int segs = 1; segs <= n_rad; ++segs) {
       const int seg = (n_rad + segs - 1) / segs;
-      if (seg < 2 * wpad && segs > 1) break;
+      if (seg < min_seg && segs > 1) break;
       const int real_segs = (n_rad + seg - 1) / seg;
       const long long ctas = (long long)chan_blocks * real_segs;
       const long long waves = (ctas + slots - 1) / slots;
