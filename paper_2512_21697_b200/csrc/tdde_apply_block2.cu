@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(B2_NC, (W <= 3 ? 4 : W <= 6 ? B2_MINB6 : 2)) k
   const int i0 = blockIdx.y * p.seg_len, i1 = min(n_rad, i0 + p.seg_len);
   const int jlo = max(0, i0 - W), jhi = min(n_rad, i1 + W), jend = i1 + W;
   const int nchunks = (jend - jlo + JC - 1) / JC;
-  const int slot = p.slot[ac];
+  const int slot = p.slot[ac] < p.n_cta_cls ? p.slot[ac] : -1;   // classes beyond the staged ones: coefficients from global (L1 / L2)
   const size_t cls_off = (size_t)p.cls[ac] * n_rad * ND;
   const int* cta_cls = p.cta_cls + blockIdx.x * B2_MAXC;
   const int nch = min(B2_NC, ld - a0);                        // channels of this CTA inside the vector
@@ -88,12 +88,12 @@ __global__ void __launch_bounds__(B2_NC, (W <= 3 ? 4 : W <= 6 ? B2_MINB6 : 2)) k
     if (nr <= 0) return;
     int ncls = 0;
 #pragma unroll
-    for (int q = 0; q < B2_MAXC; ++q) ncls += (cta_cls[q] >= 0);
+    for (int q = 0; q < B2_MAXC; ++q) ncls += (q < p.n_cta_cls && cta_cls[q] >= 0);
     const bool x2d = p.use_xmap != 0;                           // one tensor copy for the x rows: full box, out-of-bounds zero-filled
     b2_expect_tx(bar, (uint32_t)((2 * ncls * nr * ND + (x2d ? JC * B2_NC : nr * nch)) * sizeof(cplx)));
 #pragma unroll
     for (int q = 0; q < B2_MAXC; ++q) {
-      const int kk = cta_cls[q];
+      const int kk = q < p.n_cta_cls ? cta_cls[q] : -1;
       if (kk >= 0) {
         b2_bulk(st + (size_t)q * JC * ND, p.blk + ((size_t)kk * n_rad + j) * ND, (uint32_t)nr * ND * sizeof(cplx), bar);
         b2_bulk(st + CS + (size_t)q * JC * ND, blk2 + ((size_t)kk * n_rad + j) * ND, (uint32_t)nr * ND * sizeof(cplx), bar);
