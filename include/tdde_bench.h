@@ -51,6 +51,11 @@ int tdde_selftest_partition(int32_t n, int32_t w, int32_t P, uint32_t seed, doub
  * 3 = k_apply_mma (banded path, radial contraction on the FP64 tensor-core path). */
 int tdde_iter_apply_kernel(const tdde_handle* h);
 
+/* Host-only self-test of the operand table behind k_apply_mma (no GPU needed): random column bands R_L of half-bandwidth w (3, 6 or 9)
+ * and size n_rad, T terms; builds the MMA fragment table, replays the kernel's slice / tile / three-product arithmetic on the host for
+ * one channel and writes max_i |y_i - sum_L (R_L z_L)_i| / max_i |.| to *max_rel_err (host). */
+int tdde_selftest_mma_frags(int32_t n_rad, int32_t w, int32_t T, uint32_t seed, double* max_rel_err);
+
 /* Number of kernels this handle has launched since creation (bench.py's gpu_launches). */
 int64_t tdde_launch_count(const tdde_handle* h);
 

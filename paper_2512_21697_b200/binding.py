@@ -19,7 +19,7 @@ LIB_PATH = os.environ.get("TDDE_LIB_PATH", os.path.join(_HERE, "libtdde.so"))
 EXPORTS = [
     "tdde_create", "tdde_step", "tdde_propagate", "tdde_norm", "tdde_apply", "tdde_precond",
     "tdde_propagate_host", "tdde_step_forced", "tdde_apply_coupling", "tdde_time_kernel", "tdde_fp64_peak", "tdde_launch_count",
-    "tdde_apply_path", "tdde_iter_apply_kernel", "tdde_nccl_unique_id", "tdde_group_create", "tdde_group_propagate", "tdde_group_destroy", "tdde_set_eigenstates", "tdde_project", "tdde_eigensolve", "tdde_selftest_partition", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
+    "tdde_apply_path", "tdde_iter_apply_kernel", "tdde_nccl_unique_id", "tdde_group_create", "tdde_group_propagate", "tdde_group_destroy", "tdde_set_eigenstates", "tdde_project", "tdde_eigensolve", "tdde_selftest_partition", "tdde_selftest_mma_frags", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
 ]
 
 STATUS = {0: "TDDE_OK", -1: "TDDE_EINVAL", -2: "TDDE_ENOMEM", -3: "TDDE_ECUDA", -4: "TDDE_ESINGULAR",
@@ -99,6 +99,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.tdde_eigensolve.restype = C.c_int
     lib.tdde_selftest_partition.argtypes = [i32, i32, i32, C.c_uint32, C.POINTER(dbl)]
     lib.tdde_selftest_partition.restype = C.c_int
+    lib.tdde_selftest_mma_frags.argtypes = [i32, i32, i32, C.c_uint32, C.POINTER(dbl)]
+    lib.tdde_selftest_mma_frags.restype = C.c_int
     lib.tdde_paper_variant.argtypes = [vp, vp, vp, vp, i32, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i64)]
     lib.tdde_paper_variant.restype = C.c_int
     lib.tdde_nccl_unique_id.argtypes = [vp]

@@ -478,3 +478,68 @@ int launch_apply_mma(const ApplyArgs& a, int T, int m0, int mstep, int W, cudaSt
 #undef X
   return -1;
 }
+
+// ---- host self-test of the operand table and the slice / tile arithmetic (no GPU): replays what k_apply_mma does with the fragments
+// -- slice rows 4Q - OFF + (lane % 4), tiles Q/2 + F(par) + k, B[k][n] = lane 4 n + k, the three Gauss products -- for one channel and
+// random z_L, and compares with the band product y[i] = sum_L sum_j R_L[i][j] z_L[j] taken straight from the column bands. ----
+template <int W>
+static double selftest_frags_w(int T, int n_rad, const std::vector<std::complex<double>>& Rall, const std::vector<std::complex<double>>& z) {
+  using G = MmaGrid<W>;
+  constexpr int ND = 2 * W + 1;
+  std::vector<double> fr;
+  build_frags_w<W>(T, n_rad, Rall.data(), fr);
+  const int ntile = (n_rad + 7) / 8, nQ = 2 * (ntile - 1) + G::C0 + 1;
+  const size_t per = (size_t)T * (G::NTL(0) + G::NTL(1)) * 96;
+  std::vector<double> A1((size_t)ntile * 8, 0.0), A2(A1), A3(A1);
+  for (int Q = 0; Q < nQ; ++Q) {
+    const int par = Q & 1, u = Q >> 1;
+    const double* base = fr.data() + per * u + (par ? (size_t)T * G::NTL(0) * 96 : 0);
+    for (int L = 0; L < T; ++L)
+      for (int k = 0; k < G::NTL(par); ++k) {
+        const int tile = u + G::F(par) + k;
+        if (tile < 0 || tile >= ntile) continue;
+        const double* f = base + ((size_t)L * G::NTL(par) + k) * 96;
+        for (int n = 0; n < 8; ++n)
+          for (int kk = 0; kk < 4; ++kk) {
+            const int j = 4 * Q - G::OFF + kk;
+            const std::complex<double> zz = (j >= 0 && j < n_rad) ? z[(size_t)L * n_rad + j] : std::complex<double>(0, 0);
+            const int lane = 4 * n + kk;
+            A1[(size_t)tile * 8 + n] += zz.real() * f[lane];
+            A2[(size_t)tile * 8 + n] += (zz.imag() - zz.real()) * f[32 + lane];
+            A3[(size_t)tile * 8 + n] += (zz.real() + zz.imag()) * f[64 + lane];
+          }
+      }
+  }
+  double err = 0, nrm = 0;
+  for (int i = 0; i < n_rad; ++i) {
+    std::complex<double> ref(0, 0);
+    for (int L = 0; L < T; ++L)
+      for (int j = std::max(0, i - W); j <= std::min(n_rad - 1, i + W); ++j) ref += Rall[((size_t)j * T + L) * ND + (i - j + W)] * z[(size_t)L * n_rad + j];
+    const std::complex<double> got(A1[i] - A3[i], A1[i] + A2[i]);
+    err = std::max(err, std::abs(got - ref));
+    nrm = std::max(nrm, std::abs(ref));
+  }
+  return nrm > 0 ? err / nrm : err;
+}
+
+#ifdef TDDE_WITH_BENCH
+extern "C" int tdde_selftest_mma_frags(int32_t n_rad, int32_t w, int32_t T, uint32_t seed, double* max_rel_err) {
+  if (n_rad < 1 || T < 1 || !max_rel_err) return TDDE_EINVAL;
+  const int ND = 2 * w + 1;
+  std::vector<std::complex<double>> Rall((size_t)n_rad * T * ND), z((size_t)T * n_rad);
+  uint64_t s = seed * 2654435761u + 12345u;
+  auto rnd = [&]() { s = s * 6364136223846793005ull + 1442695040888963407ull; return (double)((s >> 11) & 0xFFFFFFFFu) / 4294967296.0 - 0.5; };
+  for (auto& v : Rall) v = {rnd(), rnd()};
+  for (auto& v : z) v = {rnd(), rnd()};
+  // entries of a column band that point outside the matrix must not matter: poison them
+  for (int j = 0; j < n_rad; ++j)
+    for (int L = 0; L < T; ++L)
+      for (int e = 0; e < ND; ++e) { const int i = j - w + e; if (i < 0 || i >= n_rad) Rall[((size_t)j * T + L) * ND + e] = {1e30, -1e30}; }
+  switch (w) {
+    case 3: *max_rel_err = selftest_frags_w<3>(T, n_rad, Rall, z); return 0;
+    case 6: *max_rel_err = selftest_frags_w<6>(T, n_rad, Rall, z); return 0;
+    case 9: *max_rel_err = selftest_frags_w<9>(T, n_rad, Rall, z); return 0;
+    default: return TDDE_EINVAL;
+  }
+}
+#endif

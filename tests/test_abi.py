@@ -137,6 +137,16 @@ def test_partitioned_factorisation_host(lib, n, w, P):
     assert res.value < 1e-13, (n, w, P, used, res.value)
 
 
+@pytest.mark.parametrize("n_rad,w,T", [(8, 3, 1), (37, 3, 7), (64, 6, 5), (101, 6, 7), (50, 9, 7), (19, 9, 2), (7, 6, 3)])
+def test_mma_operand_table_host(lib, n_rad, w, T):
+    """Host replay of k_apply_mma's radial contraction (tdde_apply_mma.cu: 4-row slices, 8-row tiles, B-operand fragments in lane
+    order, complex product by three real ones) against the band product taken from the column bands: radial sizes that are not
+    multiples of 8 or 4, sizes smaller than the band, all three instantiated bandwidths; out-of-matrix band entries are poisoned."""
+    res = C.c_double()
+    assert lib.tdde_selftest_mma_frags(n_rad, w, T, 11, C.byref(res)) == 0
+    assert res.value < 1e-13, (n_rad, w, T, res.value)
+
+
 def test_reference_arm_prints_on_rank0_only():
     """bench.py --impl reference under a 2-rank launch: rank 0 prints the JSON line, other ranks exit 0 silently."""
     import json
