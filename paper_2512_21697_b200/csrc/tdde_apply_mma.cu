@@ -24,10 +24,17 @@
 #include <type_traits>
 #include "tdde_reduce.cuh"
 
-#ifndef MM_NC
-#define MM_NC 96             // channels per CTA (8 channels per warp): 12 warps, one CTA per SM, <= 168 registers
+// Channels per CTA (8 per warp), chosen per bandwidth from measurements on B200 (HBM-scale / Large in-iteration apply):
+//   W = 6: 128 channels = 16 warps at <= 128 registers, the addv / aux rows loaded when a tile is emitted: 1.552 / 0.227 ms
+//          (96 channels = 12 warps at <= 168 registers with those rows prefetched one period ahead: 1.575 / 0.235 ms)
+//   W = 9: 96 channels with the prefetch: 1.93 ms (128 channels: the accumulators of 4-5 live tiles spill, 2.40 ms)
+#ifndef MM_NC6
+#define MM_NC6 128
 #endif
-#define MM_NT (MM_NC * 4)
+#ifndef MM_NC9
+#define MM_NC9 96
+#endif
+__host__ __device__ constexpr int mm_nc(int W) { return W <= 6 ? MM_NC6 : MM_NC9; }
 #ifndef MM_NSTAGE
 #define MM_NSTAGE 6          // pipeline stages wanted (fewer when shared memory is short)
 #endif
@@ -84,17 +91,19 @@ struct MmaPlan {
   using G = MmaGrid<W>;
   using SH = MmaShape<T, M0, MS>;
   static constexpr int MAXM = SH::maxm();
-  static constexpr int XW = MM_NC + 2 * MAXM;
+  static constexpr int NC = mm_nc(W), NT = 4 * NC;
+  static constexpr bool PF = NC <= 96;                              // prefetch the addv / aux rows of the next tile into registers
+  static constexpr int XW = NC + 2 * MAXM;
   // row pitch of the x tile: = 2 or 6 (mod 8) complex, so the 4 rows x 2 channels of a quarter-warp hit all 32 banks once
   __host__ __device__ static constexpr int pitch() { int p = XW; while (p % 8 != 2 && p % 8 != 6) ++p; return p; }
   static constexpr int XP = pitch();
   static constexpr int FR0 = T * G::NTL(0) * 96, FR1 = T * G::NTL(1) * 96;      // doubles per slice of parity 0 / 1
   static constexpr int FRMAX = FR0 > FR1 ? FR0 : FR1;
   static constexpr int STAGE_BYTES = FRMAX * 8 + 4 * XP * 16;
-  // the last NAS terms (the widest) keep beta g_L A_L in shared memory [slot][64 channels]; the others in registers
+  // the last NAS terms (the widest) keep beta g_L A_L in shared memory [slot][NC channels]; the others in registers
   static constexpr int NAS = (T >= 7) ? MM_ASMEM : MM_ASMEM5;
   static constexpr int NSREG = SH::slot0(T - NAS);                  // register slots
-  static constexpr int AS_BYTES = (SH::nslots() - NSREG) * MM_NC * 16;
+  static constexpr int AS_BYTES = (SH::nslots() - NSREG) * NC * 16;
   __host__ __device__ static constexpr int stages() {
     int n = (226 * 1024 - AS_BYTES - 256) / STAGE_BYTES;
     return n > MM_NSTAGE ? MM_NSTAGE : n;
@@ -135,11 +144,11 @@ __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
 }
 
 template <int T, int M0, int MS, int W>
-__global__ void __launch_bounds__(MM_NT, 1) k_apply_mma(const __grid_constant__ ApplyArgs p) {
+__global__ void __launch_bounds__(4 * mm_nc(W), 1) k_apply_mma(const __grid_constant__ ApplyArgs p) {
   using PL = MmaPlan<T, M0, MS, W>;
   using G = MmaGrid<W>;
   using SH = MmaShape<T, M0, MS>;
-  constexpr int MAXM = PL::MAXM, XP = PL::XP, NS = SH::nslots(), NL = G::NLIVE();
+  constexpr int MAXM = PL::MAXM, XP = PL::XP, NS = SH::nslots(), NL = G::NLIVE(), MM_NC = PL::NC, MM_NT = PL::NT;
   if (p.guard == 1 && solver_idle(p.red.st)) return;
   if (p.guard == 2 && (p.red.st->stalled | (p.red.st->status != 0))) return;
 
@@ -228,9 +237,7 @@ __global__ void __launch_bounds__(MM_NT, 1) k_apply_mma(const __grid_constant__ 
       }
     }
   };
-#ifndef MM_NOPF
-  prefetch(0);
-#endif
+  if (PL::PF) prefetch(0);
   __syncthreads();                                              // As visible to the whole warp
   cplx d0 = make_double2(0, 0);
   double d1 = 0;
@@ -299,9 +306,7 @@ __global__ void __launch_bounds__(MM_NT, 1) k_apply_mma(const __grid_constant__ 
   auto emit = [&](int u) {                                         // tile u - EV is complete: combine, add, store, inner products
     const int v = u - G::EV;
     if (v >= 0 && v < ntile) {
-#ifdef MM_NOPF
-      prefetch(v);
-#endif
+      if (!PL::PF) prefetch(v);
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
         const int i = i0 + 8 * v + 2 * r + e;
@@ -325,9 +330,7 @@ __global__ void __launch_bounds__(MM_NT, 1) k_apply_mma(const __grid_constant__ 
       for (int e = 0; e < 3; ++e) { acc[k][e][0] = acc[k + 1][e][0]; acc[k][e][1] = acc[k + 1][e][1]; }
 #pragma unroll
     for (int e = 0; e < 3; ++e) { acc[NL - 1][e][0] = 0; acc[NL - 1][e][1] = 0; }
-#ifndef MM_NOPF
-    if (v + 1 < ntile) prefetch(v + 1);
-#endif
+    if (PL::PF && v + 1 < ntile) prefetch(v + 1);
   };
   using I0 = std::integral_constant<int, 0>;
   using I1 = std::integral_constant<int, 1>;
@@ -444,7 +447,7 @@ bool build_mma_frags(int T, int W, int n_rad, const void* Rall, std::vector<doub
   }
 }
 
-int apply_mma_channels() { return MM_NC; }
+int apply_mma_channels(int W) { return mm_nc(W); }
 
 int apply_mma_halo(int W) {     // input rows a segment reads beyond its own, both ends together (for the segment-length choice)
   switch (W) {
@@ -465,14 +468,15 @@ static int launch_mma_one(const ApplyArgs& a, dim3 grid, cudaStream_t s) {
     if (cudaFuncSetAttribute(k_apply_mma<T, M0, MS, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -2;
     if (dev >= 0 && dev < 64) attr_set[dev] = true;
   }
-  k_apply_mma<T, M0, MS, W><<<grid, MM_NT, smem, s>>>(a);
+  k_apply_mma<T, M0, MS, W><<<grid, 4 * mm_nc(W), smem, s>>>(a);
   return 1;
 }
 
 // y = addv + (coupling terms) x with fused <aux, y>, ||y||^2; a.seg_len must be a multiple of 8
 int launch_apply_mma(const ApplyArgs& a, int T, int m0, int mstep, int W, cudaStream_t s) {
   if (!a.addv || !a.Rfrag || (a.emode != 0 && a.emode != 3) || (a.emode == 3 && (!a.aux || !a.y2)) || (a.seg_len & 7)) return -1;
-  dim3 grid((a.ld + MM_NC - 1) / MM_NC, (a.n_rad + a.seg_len - 1) / a.seg_len);
+  const int nc = mm_nc(W);
+  dim3 grid((a.ld + nc - 1) / nc, (a.n_rad + a.seg_len - 1) / a.seg_len);
 #define X(t, aa, b, w) if (T == t && m0 == aa && mstep == b && W == w) return launch_mma_one<t, aa, b, w>(a, grid, s);
   TDDE_MMA_SHAPES(X)
 #undef X

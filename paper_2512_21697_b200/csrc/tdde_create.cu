@@ -424,7 +424,7 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
       std::vector<double> frags;
       if (build_mma_frags(T, h->bW, n_rad, Rall.data(), frags)) {
         if ((rc = dev_upload(&h->d_Rfrag, frags.data(), frags.size(), s))) return rc;
-        const int nc = apply_mma_channels(), chan_blocks = (h->ld + nc - 1) / nc, halo = apply_mma_halo(h->bW);
+        const int nc = apply_mma_channels(h->bW), chan_blocks = (h->ld + nc - 1) / nc, halo = apply_mma_halo(h->bW);
         long long best_cost = -1;
         int best_seg = (n_rad + 7) / 8 * 8;
         for (int seg = 8; seg <= (n_rad + 7) / 8 * 8; seg += 8) {

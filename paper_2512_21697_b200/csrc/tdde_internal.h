@@ -187,7 +187,7 @@ int launch_apply_generic(const ApplyArgs& a, int num_sms, cudaStream_t s);
 // DMMA variant of the in-iteration banded apply (y = addv + coupling terms): shapes, fragment table, launcher
 bool apply_mma_available(int T, int m0, int mstep, int W);
 int apply_mma_halo(int W);
-int apply_mma_channels();
+int apply_mma_channels(int W);
 int launch_apply_mma(const ApplyArgs& a, int T, int m0, int mstep, int W, cudaStream_t s);
 int launch_block_dual(const ApplyArgs& a, const cplx* blk2, int W, cudaStream_t s);   // y = oscale (blk) x, y2 = (blk2) x
 int launch_apply_sparse(const ApplyArgs& a, int W, cudaStream_t s);
