@@ -229,6 +229,51 @@ def whole_job_rate(world: int, steps: int, max_ms: float) -> float:
     return world * steps / (max_ms * 1e-3)
 
 
+# ------------------------------------------------------------------------------ NEXT-3: channel-slab shards on one GPU
+def sharded_main(args):
+    """--shards N: the lock-step sharded driver (tdde_group_*) with all N shards in this process on ONE GPU, next to the
+    unsharded propagation of the same problem.  It measures the overhead of the sharded driver (halo copies, split reductions, one
+    host read per step, halo recomputation), NOT scaling: the pool has one-GPU boxes."""
+    import torch
+    from paper_2512_21697_b200 import Tdde, TddeGroup, sharding
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device")
+    K, W, N = args.steps, max(args.warmup, 3), args.shards
+    p = load_problem(args.config, args.phase, args.e0)
+    g_all = p.g_table(W + K)
+    prop = Tdde(p)
+    c = prop.to_device(p.c0)
+    prop.propagate(c, g_all[:W])
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); st1 = prop.propagate(c, g_all[W:W + K]); e1.record(); torch.cuda.synchronize()
+    ms1 = e0.elapsed_time(e1)
+    c_ref = c.cpu().numpy().reshape(p.n_ang, p.n_rad)
+    prop.close(); del c
+    parts = sharding.shard_specs(p, N)
+    shards = [Tdde(pl) for _, pl, _ in parts]
+    grp = TddeGroup(shards, [sp for _, _, sp in parts])
+    c0 = p.c0.reshape(p.n_ang, p.n_rad)
+    cs = [sh.to_device(np.ascontiguousarray(c0[pl.halo_lo:pl.halo_hi]).reshape(-1)) for (pl, _, _), sh in zip(parts, shards)]
+    grp.propagate(cs, g_all[:W])
+    e0.record(); st = grp.propagate(cs, g_all[W:W + K]); e1.record(); torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    err2 = ref2 = 0.0
+    for (pl, _, _), cd in zip(parts, cs):
+        own = cd.cpu().numpy().reshape(pl.n_local, p.n_rad)[pl.own_slice]
+        err2 += float(np.sum(np.abs(own - c_ref[pl.lo:pl.hi]) ** 2)); ref2 += float(np.sum(np.abs(c_ref[pl.lo:pl.hi]) ** 2))
+    print(json.dumps({"metric": METRIC, "value": K / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms / K,
+                      "higher_is_better": True, "impl": "ours-sharded", "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": args.config, "n_ang": p.n_ang, "n_rad": p.n_rad, "n_terms": p.n_terms,
+                                 "parallelism": "%d channel-slab shards in ONE process on 1 GPU (lock-step driver: overhead, not scaling)" % N,
+                                 "halo_channels_per_side": parts[0][0].reach},
+                      "half_iters_per_step": st["half_iters"] / K, "unsharded_ms_per_step": ms1 / K,
+                      "unsharded_half_iters_per_step": st1["half_iters"] / K, "overhead": ms / ms1 - 1.0,
+                      "rel_diff_vs_unsharded": (err2 / ref2) ** 0.5}))
+    grp.close()
+    for sh in shards:
+        sh.close()
+
+
 # ----------------------------------------------------------------------------------------------------- our arm
 def ours_main(args):
     import torch
@@ -383,11 +428,15 @@ def main():
     ap.add_argument("--kernel-reps", type=int, default=10)
     ap.add_argument("--sample-ang", type=int, default=24, help="angular channels of the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shards", type=int, default=0, help="N >= 2: run the channel-slab sharded driver with N shards in this process on one "
+                    "GPU next to the unsharded run (DESIGN.md 7: driver overhead, not scaling)")
     ap.add_argument("--paper-variant", action="store_true",
                     help="also time the paper's formulation (CSR assembly + SpMV) on this GPU; needs 20 B per non-zero")
     args = ap.parse_args()
     if args.impl == "reference":
         reference_main(args)
+    elif args.shards >= 2:
+        sharded_main(args)
     else:
         ours_main(args)
 
