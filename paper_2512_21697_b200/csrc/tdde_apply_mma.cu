@@ -143,7 +143,9 @@ __device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
 }
 
-template <int T, int M0, int MS, int W>
+// GATHER (channel-slab shards, tdde_shard.cu): the halo columns of the x tile are fetched by the TMA producer straight from the vectors of
+// the neighbouring shards (p.xL / p.xR: same device, or peer memory), so no halo copy precedes the apply
+template <int T, int M0, int MS, int W, bool GATHER>
 __global__ void __launch_bounds__(4 * mm_nc(W), 1) k_apply_mma(const __grid_constant__ ApplyArgs p) {
   using PL = MmaPlan<T, M0, MS, W>;
   using G = MmaGrid<W>;
@@ -183,6 +185,13 @@ __global__ void __launch_bounds__(4 * mm_nc(W), 1) k_apply_mma(const __grid_cons
   __syncthreads();
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 
+  // GATHER: [xa_lo, xa_hi) = [left halo | owned | right halo]: three sources, the same bytes in total (set up once per CTA)
+  const int gc1 = GATHER ? min(xa_hi, max(xa_lo, p.own_lo)) : xa_lo, gc2 = GATHER ? min(xa_hi, max(gc1, p.own_hi)) : xa_hi;
+  const cplx* gsL = (GATHER && p.xL) ? p.xL + xa_lo + p.shiftL : p.x + xa_lo;
+  const cplx* gsR = (GATHER && p.xR) ? p.xR + gc2 + p.shiftR : p.x + gc2;
+  const int gldL = (GATHER && p.xL) ? p.ldL : ld, gldR = (GATHER && p.xR) ? p.ldR : ld;
+  const uint32_t gbL = (uint32_t)(gc1 - xa_lo) * sizeof(cplx), gbO = (uint32_t)(gc2 - gc1) * sizeof(cplx), gbR = (uint32_t)(xa_hi - gc2) * sizeof(cplx);
+  const int gcO = gc1, gdO = gc1 - xa_lo, gdR = gc2 - xa_lo;
   auto issue = [&](int q) {                                    // one thread: the bulk copies of slice q
     unsigned char* st = smem_raw + (size_t)(q % PL::NSTAGE) * PL::STAGE_BYTES;
     uint64_t* bar = &full[q % PL::NSTAGE];
@@ -195,8 +204,19 @@ __global__ void __launch_bounds__(4 * mm_nc(W), 1) k_apply_mma(const __grid_cons
     const double* fsrc = p.Rfrag + (size_t)((Q0 + q) >> 1) * (PL::FR0 + PL::FR1) + (par ? PL::FR0 : 0);
     mm_bulk_g2s(st, fsrc, fbytes, bar);
     cplx* xs = reinterpret_cast<cplx*>(st + PL::FRMAX * 8);
-    for (int rr = 0; rr < 4; ++rr)
-      if (j0 + rr >= 0 && j0 + rr < n_rad) mm_bulk_g2s(xs + rr * XP + x_dst_off, p.x + (size_t)(j0 + rr) * ld + xa_lo, x_bytes, bar);
+    if (!GATHER) {
+      for (int rr = 0; rr < 4; ++rr)
+        if (j0 + rr >= 0 && j0 + rr < n_rad) mm_bulk_g2s(xs + rr * XP + x_dst_off, p.x + (size_t)(j0 + rr) * ld + xa_lo, x_bytes, bar);
+    } else {
+      for (int rr = 0; rr < 4; ++rr) {
+        const int j = j0 + rr;
+        if (j < 0 || j >= n_rad) continue;
+        cplx* dst = xs + rr * XP + x_dst_off;
+        if (gbL) mm_bulk_g2s(dst, gsL + (size_t)j * gldL, gbL, bar);
+        if (gbO) mm_bulk_g2s(dst + gdO, p.x + (size_t)j * ld + gcO, gbO, bar);
+        if (gbR) mm_bulk_g2s(dst + gdR, gsR + (size_t)j * gldR, gbR, bar);
+      }
+    }
   };
   if (tid == 0)
     for (int q = 0; q < PL::NSTAGE && q < nq; ++q) issue(q);
@@ -458,17 +478,17 @@ int apply_mma_halo(int W) {     // input rows a segment reads beyond its own, bo
   }
 }
 
-template <int T, int M0, int MS, int W>
+template <int T, int M0, int MS, int W, bool GATHER>
 static int launch_mma_one(const ApplyArgs& a, dim3 grid, cudaStream_t s) {
   static bool attr_set[64] = {};
   const size_t smem = MmaPlan<T, M0, MS, W>::SMEM;
   int dev = 0;
   cudaGetDevice(&dev);
   if (dev < 0 || dev >= 64 || !attr_set[dev]) {
-    if (cudaFuncSetAttribute(k_apply_mma<T, M0, MS, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -2;
+    if (cudaFuncSetAttribute(k_apply_mma<T, M0, MS, W, GATHER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return -2;
     if (dev >= 0 && dev < 64) attr_set[dev] = true;
   }
-  k_apply_mma<T, M0, MS, W><<<grid, 4 * mm_nc(W), smem, s>>>(a);
+  k_apply_mma<T, M0, MS, W, GATHER><<<grid, 4 * mm_nc(W), smem, s>>>(a);
   return 1;
 }
 
@@ -477,7 +497,9 @@ int launch_apply_mma(const ApplyArgs& a, int T, int m0, int mstep, int W, cudaSt
   if (!a.addv || !a.Rfrag || (a.emode != 0 && a.emode != 3) || (a.emode == 3 && (!a.aux || !a.y2)) || (a.seg_len & 7)) return -1;
   const int nc = mm_nc(W);
   dim3 grid((a.ld + nc - 1) / nc, (a.n_rad + a.seg_len - 1) / a.seg_len);
-#define X(t, aa, b, w) if (T == t && m0 == aa && mstep == b && W == w) return launch_mma_one<t, aa, b, w>(a, grid, s);
+#define X(t, aa, b, w)                                                 \
+  if (T == t && m0 == aa && mstep == b && W == w)                      \
+    return (a.xL || a.xR) ? launch_mma_one<t, aa, b, w, true>(a, grid, s) : launch_mma_one<t, aa, b, w, false>(a, grid, s);
   TDDE_MMA_SHAPES(X)
 #undef X
   return -1;

@@ -55,6 +55,17 @@ int enqueue_apply(tdde_handle* h, const cplx* x, cplx* y, const cplx* aux, int b
     if (a.addv && T > 0 && (emode == 0 || emode == 3) && h->seg_len_m > 0) {      // y = addv + coupling terms: DMMA variant
       a.Rfrag = h->d_Rfrag;
       a.seg_len = h->seg_len_m;
+      if (h->nbrL || h->nbrR) {                                   // sharded: halo columns straight from the neighbours' copy of this vector
+        const cplx* mine[9] = {h->X, h->r, h->rhat, h->p, h->v, h->s, h->t, h->y, h->z};
+        int idx = -1;
+        for (int q = 0; q < 9; ++q) if (mine[q] == x) idx = q;
+        auto pick = [&](tdde_handle* n) -> const cplx* {
+          const cplx* theirs[9] = {n->X, n->r, n->rhat, n->p, n->v, n->s, n->t, n->y, n->z};
+          return theirs[idx];
+        };
+        if (idx >= 0 && h->nbrL) { a.xL = pick(h->nbrL); a.ldL = h->nbrL->ld; a.shiftL = h->shiftL; }
+        if (idx >= 0 && h->nbrR) { a.xR = pick(h->nbrR); a.ldR = h->nbrR->ld; a.shiftR = h->shiftR; }
+      }
       rc = launch_apply_mma(a, T, h->bM0, h->bMS, h->bW, h->stream);
       if (rc == -1) a.seg_len = h->seg_len;
     }

@@ -75,6 +75,10 @@ struct tdde_handle {
   // [own_lo, own_hi) (the rest are halo inputs) and hands its reduction sums to the group instead of finalising them
   int own_lo = 0, own_hi = 0;                // own_hi == 0: not sharded (all of [0, ld))
   double* shard_sums = nullptr;              // device [4]
+  // fused halo gather (k_apply_mma<GATHER>): the shards that own this shard's left / right halo columns and the channel shift into
+  // their local numbering; set by tdde_group_create when every shard of the process qualifies
+  tdde_handle *nbrL = nullptr, *nbrR = nullptr;
+  int shiftL = 0, shiftR = 0;
 
   // solver state, scratch
   SolverState* d_st = nullptr;

@@ -136,6 +136,9 @@ struct ApplyArgs {
   const cplx* blk_row;     // row-band block coefficients [n_cls][n_rad][2w0+1]
   int w[TDDE_MAX_TERMS];
   int w0;
+  // k_apply_mma<GATHER> (sharding): channel a < own_lo of row j is xL[j * ldL + a + shiftL], a >= own_hi is xR[j * ldR + a + shiftR]
+  const cplx *xL, *xR;
+  int ldL, ldR, shiftL, shiftR;
   int own_lo, own_hi;      // channels [own_lo, own_hi) are written and enter the fused sums (sharding: the owned slab; else 0, ld)
   int guard;               // 0 none; 1: no-op when st->done|stalled|status (iterations); 2: no-op when stalled|status (start of step)
   ReduceCtx red;

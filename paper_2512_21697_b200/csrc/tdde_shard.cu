@@ -11,6 +11,7 @@
 // r, rhat, p, v, s, t therefore stay exactly zero (they are zero at attach and every update of them is linear in them), so the
 // vector kernels need no mask.  The host reads the solver state once per CN step (the single-GPU driver: once per 64 steps).
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 #include <vector>
 #include <dlfcn.h>
@@ -71,6 +72,7 @@ struct tdde_group {
   int world = 1;
   void* comm = nullptr;            // ncclComm_t, or nullptr: all shards local
   double** d_bufptr = nullptr;     // device array of the local shards' sum buffers (local all-reduce)
+  bool gather = false;             // the in-iteration applies fetch their halo columns themselves (k_apply_mma<GATHER>): no copies for y, z
   cudaStream_t stream = nullptr;
 };
 
@@ -105,6 +107,7 @@ static int copy_grid(long long tot) { return (int)std::max<long long>(1, std::mi
 
 // refresh the halo columns of vector v on every local shard
 static int group_exchange(tdde_group* g, int v) {
+  if (g->gather && v != SV_X) return 0;                      // gathered inside the apply
   cudaStream_t s = g->stream;
   NcclApi* nc = g->comm ? nccl_api() : nullptr;
   if (!g->comm) {
@@ -226,7 +229,7 @@ extern "C" void tdde_group_destroy(tdde_group* g) {
   for (size_t k = 0; k < g->hs.size(); ++k) {
     tdde_handle* h = g->hs[k];
     if (h->shard_sums) cudaFree(h->shard_sums);
-    h->shard_sums = nullptr; h->own_lo = 0; h->own_hi = 0;
+    h->shard_sums = nullptr; h->own_lo = 0; h->own_hi = 0; h->nbrL = h->nbrR = nullptr; h->shiftL = h->shiftR = 0;
     if (g->info[k].sendbuf) cudaFree(g->info[k].sendbuf);
     if (g->info[k].recvbuf) cudaFree(g->info[k].recvbuf);
   }
@@ -297,6 +300,30 @@ extern "C" int tdde_group_create(tdde_group** out, int32_t n_local, tdde_handle*
           if (g->info[q].rank == pc.peer && pc.src_lo >= g->info[q].own_lo && pc.src_lo + pc.n <= g->info[q].own_hi) ok = true;
         if (!ok) return fail(TDDE_EINVAL);
       }
+    // Fused gather: every shard runs k_apply_mma in the iteration and has at most one neighbour per side that owns its whole halo
+    bool gather = !std::getenv("TDDE_NO_GATHER") && g->hs.size() > 1;
+    for (size_t k = 0; k < g->hs.size() && gather; ++k) {
+      tdde_handle* h = g->hs[k];
+      const ShardInfo& in = g->info[k];
+      if (h->path != 1 || h->seg_len_m <= 0 || !h->use_subst || h->cfg.n_terms == 0 || in.recv.size() > 2) gather = false;
+      int nl = 0, nr = 0;
+      for (const HaloPiece& pc : in.recv) {
+        if (pc.lo == 0 && pc.n == in.own_lo) ++nl;
+        else if (pc.lo == in.own_hi && pc.lo + pc.n == h->cfg.n_ang) ++nr;
+        else gather = false;
+      }
+      if (nl > 1 || nr > 1) gather = false;
+    }
+    if (gather) {
+      for (size_t k = 0; k < g->hs.size(); ++k)
+        for (const HaloPiece& pc : g->info[k].recv) {
+          tdde_handle* src = nullptr;
+          for (size_t q = 0; q < g->hs.size(); ++q) if (g->info[q].rank == pc.peer) src = g->hs[q];
+          if (pc.lo == 0) { g->hs[k]->nbrL = src; g->hs[k]->shiftL = pc.src_lo - pc.lo; }
+          else { g->hs[k]->nbrR = src; g->hs[k]->shiftR = pc.src_lo - pc.lo; }
+        }
+      g->gather = true;
+    }
     std::vector<double*> ptrs;
     for (tdde_handle* h : g->hs) ptrs.push_back(h->shard_sums);
     if (cudaMalloc((void**)&g->d_bufptr, ptrs.size() * sizeof(double*)) != cudaSuccess) return fail(TDDE_ENOMEM);

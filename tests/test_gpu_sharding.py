@@ -43,8 +43,13 @@ def _run_sharded(p, world, n_steps, nccl=False):
     return out.reshape(-1), st
 
 
-@pytest.mark.parametrize("n_ang,T,bw,world", [(70, 3, 7, 2), (150, 7, 13, 3), (97, 5, 13, 2), (64, 7, 19, 4)])
-def test_sharded_propagation_matches_unsharded_oracle(n_ang, T, bw, world):
+@pytest.mark.parametrize("n_ang,T,bw,world,gather", [(70, 3, 7, 2, True), (150, 7, 13, 3, True), (150, 7, 13, 3, False), (97, 5, 13, 2, True),
+                                                     (64, 7, 19, 4, True), (64, 7, 19, 4, False)])
+def test_sharded_propagation_matches_unsharded_oracle(n_ang, T, bw, world, gather, monkeypatch):
+    """gather: the in-iteration applies of shards that run k_apply_mma fetch their halo columns straight from the neighbours' vectors
+    (k_apply_mma<GATHER>); TDDE_NO_GATHER=1 keeps the separate halo copies for the same problems; T = 3 has no DMMA kernel (copies)."""
+    if not gather:
+        monkeypatch.setenv("TDDE_NO_GATHER", "1")
     n_steps = 3
     p = tdde_inputs.make_synthetic(n_ang=n_ang, n_r=21, bandwidth=bw, n_terms=T, dt=0.01, n_steps=n_steps, rtol=1e-10, seed=n_ang,
                                    tiny_offsets=(T == 3), name="shard", phase=np.pi / 2, e0=1.5)
