@@ -175,6 +175,7 @@ static int enqueue_step_start(tdde_handle* h) {
     a.x = h->X; a.y = h->r; a.y2 = h->s; a.oscale = make_double2(0.0, -h->cfg.dt);
     a.n_ang = h->cfg.n_ang; a.n_rad = h->cfg.n_rad; a.ld = h->ld; a.seg_len = h->seg_len_s;
     a.cls = h->d_cls; a.blk = h->d_H0; a.slot = h->d_slot; a.cta_cls = h->d_cta_cls; a.n_cta_cls = std::min(h->cta_cls_max, 4);   // at most 4 classes staged per CTA: smaller stages, more CTAs per SM
+    if (const char* env = std::getenv("TDDE_B2_NCLS")) a.n_cta_cls = std::max(0, std::min(TDDE_AP_MAXC, std::atoi(env)));
     a.guard = 2; a.red.st = st;
     a.own_lo = h->own_lo; a.own_hi = h->own_hi > 0 ? h->own_hi : h->ld;
     if (h->have_xmaps) { a.xmap = h->xmaps[0]; a.use_xmap = 1; }      // X is work vector 0
