@@ -322,6 +322,7 @@ def ours_main(args):
     kt = {name: prop.time_kernel(which, reps, g_mid) for which, name in
           [(0, "apply"), (1, "precond"), (2, "vec_p"), (3, "vec_s"), (4, "vec_xr"), (5, "transpose"), (6, "apply_S")]}
     fp64_peak_meas = prop.fp64_peak()
+    dmma_peak_meas, mixed_peak_meas = prop.fp64_pipe_probe(1), prop.fp64_pipe_probe(2)
     pv = None
     if args.paper_variant and prop.apply_path == "banded":
         xv = prop.to_device(p.c0)
@@ -399,6 +400,9 @@ def ours_main(args):
                          "algorithmic_bytes_per_launch": bytes_per["apply"] * nint,
                          "peak_kind": "derived: %d SMs x 64 DFMA/clk x 2 x %.0f MHz" % (n_sm, sm_max),
                          "fp64_peak_measured_tflops": fp64_peak_meas / 1e12,
+                         "fp64_pipe_probe_tflops": {"dfma": fp64_peak_meas / 1e12, "dmma": dmma_peak_meas / 1e12,
+                                                    "dmma_dfma_mixed": mixed_peak_meas / 1e12,
+                                                    "note": "DMMA (mma.sync.m8n8k4.f64) and DFMA share one pipe on B200: one peak for both"},
                          "frac_of_measured_dfma": ach / (fp64_peak_meas / 1e12),
                          "cfma_per_element": F, "flops_per_launch": flops_apply,
                          "alg_hbm_GBps": kernels["apply"]["alg_GBps"], "hbm_peak_GBps": hbm, "hbm_peak_kind": peak_kind},

@@ -31,6 +31,9 @@ int tdde_apply_coupling(tdde_handle* h, tdde_c64 beta, const double* g, const td
  *   tdde_fp64_peak: run an unrolled independent-DFMA kernel on every SM and return achieved FLOP/s. */
 int tdde_time_kernel(tdde_handle* h, int32_t which, int32_t reps, const double* g, double* ms_out);
 int tdde_fp64_peak(void* cuda_stream, double* flops_out);
+/* The same for the pipe k_apply_mma runs on: mode 0 = DFMA only, 1 = DMMA only (mma.sync.m8n8k4.f64), 2 = 8 DMMA : 32 DFMA mixed in one warp.
+ * On B200 all three land on one peak (DMMA and DFMA share the FP64 pipe), the mix about 12 % below it. */
+int tdde_fp64_pipe_probe(void* cuda_stream, int32_t mode, double* flops_out);
 
 /* Comparator, not on the product path: the paper's own formulation on this GPU.  Allocates the global
  * CSR matrix A = S + i dt/2 H(g) (structure once), recomputes every non-zero from the stored radial and

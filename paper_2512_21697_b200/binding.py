@@ -18,7 +18,7 @@ LIB_PATH = os.environ.get("TDDE_LIB_PATH", os.path.join(_HERE, "libtdde.so"))
 
 EXPORTS = [
     "tdde_create", "tdde_step", "tdde_propagate", "tdde_norm", "tdde_apply", "tdde_precond",
-    "tdde_propagate_host", "tdde_step_forced", "tdde_apply_coupling", "tdde_time_kernel", "tdde_fp64_peak", "tdde_launch_count",
+    "tdde_propagate_host", "tdde_step_forced", "tdde_apply_coupling", "tdde_time_kernel", "tdde_fp64_peak", "tdde_fp64_pipe_probe", "tdde_launch_count",
     "tdde_apply_path", "tdde_iter_apply_kernel", "tdde_nccl_unique_id", "tdde_group_create", "tdde_group_propagate", "tdde_group_destroy", "tdde_set_eigenstates", "tdde_project", "tdde_eigensolve", "tdde_selftest_partition", "tdde_selftest_mma_frags", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
 ]
 
@@ -86,6 +86,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.tdde_apply_coupling.argtypes = [vp, tdde_c64, vp, vp, vp, vp, vp, i32, vp]
     lib.tdde_apply_coupling.restype = C.c_int
     lib.tdde_fp64_peak.argtypes = [vp, C.POINTER(dbl)]
+    lib.tdde_fp64_pipe_probe.argtypes = [vp, i32, C.POINTER(dbl)]
+    lib.tdde_fp64_pipe_probe.restype = C.c_int
     lib.tdde_launch_count.argtypes = [vp]
     lib.tdde_launch_count.restype = i64
     lib.tdde_apply_path.argtypes = [vp]
@@ -304,6 +306,12 @@ class Tdde:
                                          C.byref(ta), C.byref(ts), C.byref(nnz))
         _check(self.lib, rc, "tdde_paper_variant")
         return y, ta.value, ts.value, nnz.value
+
+    def fp64_pipe_probe(self, mode: int) -> float:
+        """FLOP/s of the FP64 pipe: mode 0 DFMA, 1 DMMA, 2 DMMA + DFMA mixed (tdde_fp64_pipe_probe)."""
+        out = C.c_double()
+        _check(self.lib, self.lib.tdde_fp64_pipe_probe(C.c_void_p(self.stream.cuda_stream), mode, C.byref(out)), "tdde_fp64_pipe_probe")
+        return out.value
 
     def fp64_peak(self) -> float:
         out = C.c_double()

@@ -209,3 +209,4 @@ int launch_to_boundary(const cplx* X, cplx* c, int n_ang, int n_rad, int ld, cud
 int launch_combine_blocks(const cplx* S, const cplx* H0, cplx alpha, cplx beta, cplx* out, long long count, cudaStream_t s);
 int launch_fill(cplx* v, long long n, unsigned seed, cudaStream_t s);
 int launch_dfma_peak(double* out, int blocks, int threads, int iters, cudaStream_t s);
+int launch_fp64_pipe_probe(double* out, int blocks, int threads, int iters, int mode, cudaStream_t s);

@@ -132,6 +132,31 @@ extern "C" int tdde_fp64_peak(void* cuda_stream, double* flops_out) {
   return 0;
 }
 
+// mode 0: DFMA only (= tdde_fp64_peak), 1: DMMA only, 2: DMMA and DFMA mixed in one warp (8 : 32, the mix of k_apply_mma)
+extern "C" int tdde_fp64_pipe_probe(void* cuda_stream, int32_t mode, double* flops_out) {
+  if (!flops_out || mode < 0 || mode > 2) return TDDE_EINVAL;
+  if (mode == 0) return tdde_fp64_peak(cuda_stream, flops_out);
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  double* d = nullptr;
+  CU(cudaMalloc((void**)&d, sizeof(double)));
+  const int blocks = tdde_num_sms() * 2, threads = 256, iters = 20000;
+  launch_fp64_pipe_probe(d, blocks, threads, 64, mode, s);
+  ScopedEvent e0, e1;
+  CU(e0.create());
+  CU(e1.create());
+  CU(cudaEventRecord(e0, s));
+  launch_fp64_pipe_probe(d, blocks, threads, iters, mode, s);
+  CU(cudaEventRecord(e1, s));
+  CU(cudaEventSynchronize(e1));
+  float ms = 0;
+  CU(cudaEventElapsedTime(&ms, e0, e1));
+  cudaFree(d);
+  const double warps = (double)blocks * threads / 32.0;
+  const double flop_per_iter = 8 * 2.0 * 256.0 + (mode == 2 ? 32 * 2.0 * 32.0 : 0.0);      // per warp
+  *flops_out = warps * (double)iters * flop_per_iter / (ms * 1e-3);
+  CU(cudaGetLastError());
+  return 0;
+}
 #endif  // TDDE_WITH_BENCH
 
 // ---- observables (Eq. 33) ----

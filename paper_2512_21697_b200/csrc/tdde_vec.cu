@@ -185,6 +185,33 @@ __global__ void __launch_bounds__(256) k_dfma_peak(double* out, int iters) {
   if (s == 123.456) out[0] = s;
 }
 
+// FP64 pipe probe (DESIGN.md 4.1 (1b)): mode 1 = DMMA only (mma.sync.m8n8k4.f64, 8 independent accumulators), mode 2 = per iteration
+// 8 DMMAs followed by 32 DFMAs in the same warp -- the mix of k_apply_mma.  One flop count for both: 2 x 256 per DMMA, 2 x 32 per DFMA.
+__global__ void __launch_bounds__(256) k_fp64_pipe_probe(double* out, int iters, int mode) {
+  double c[8][2], f[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { c[i][0] = 0; c[i][1] = 0; f[i] = i; }
+  const double a = threadIdx.x * 1e-3, b = threadIdx.x * 2e-3, m = 0.999999, k = 1e-7;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+      asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a), "d"(b));
+    if (mode == 2) {
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int i = 0; i < 8; ++i) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(f[i]) : "d"(m), "d"(k));
+    }
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += c[i][0] + c[i][1] + f[i];
+  if (s == 123.456) out[0] = s;
+}
+int launch_fp64_pipe_probe(double* out, int blocks, int threads, int iters, int mode, cudaStream_t s) {
+  k_fp64_pipe_probe<<<blocks, threads, 0, s>>>(out, iters, mode); return 1;
+}
+
 int launch_vec_p(const VecArgs& a, cudaStream_t s) { k_vec_p<<<vec_grid(a.n), VEC_NT, 0, s>>>(a); return 1; }
 int launch_vec_s(const VecArgs& a, cudaStream_t s) { k_vec_s<<<vec_grid(a.n), VEC_NT, 0, s>>>(a); return 1; }
 int launch_vec_halfexit(const VecArgs& a, cudaStream_t s) { k_vec_halfexit<<<vec_grid(a.n), VEC_NT, 0, s>>>(a); return 1; }
