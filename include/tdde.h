@@ -148,7 +148,8 @@ int tdde_eigensolve(int32_t n_cls, int32_t n_rad, int32_t w0, const tdde_c64* S_
  *   own_lo, own_hi : owned channels [own_lo, own_hi) in the shard's LOCAL numbering
  *   recv_*         : halo pieces: channels [recv_lo, recv_lo + recv_n) of this shard = channels [recv_src_lo, ...) of shard recv_rank
  *   send_*         : the same pieces seen from the owner (needed with NCCL only): channels [send_lo, send_lo + send_n) go to send_rank
- * All shards must share n_rad, n_terms, dt, rtol, max_iter.  Errors: TDDE_EINVAL, TDDE_ENOMEM, TDDE_ECUDA (also: NCCL not loadable). */
+ * While a handle is attached to a group only tdde_group_propagate may drive it (its fused reductions hand their sums to the group);
+ * tdde_group_destroy detaches it.  All shards must share n_rad, n_terms, dt, rtol, max_iter, the device and the stream.  Errors: TDDE_EINVAL, TDDE_ENOMEM, TDDE_ECUDA (also: NCCL not loadable). */
 typedef struct tdde_group tdde_group;
 typedef struct {
   int32_t rank, world;
