@@ -147,6 +147,17 @@ def test_mma_operand_table_host(lib, n_rad, w, T):
     assert res.value < 1e-13, (n_rad, w, T, res.value)
 
 
+def test_group_entry_points_reject_bad_arguments(lib):
+    """tdde_group_* / tdde_nccl_unique_id (include/tdde.h, NEXT-3): argument errors are reported before any CUDA call."""
+    g = C.c_void_p()
+    assert lib.tdde_group_create(None, 1, None, None, None) == -1
+    assert lib.tdde_group_create(C.byref(g), 0, None, None, None) == -1 and not g.value
+    assert lib.tdde_group_create(C.byref(g), 1, None, None, None) == -1 and not g.value
+    assert lib.tdde_group_propagate(None, None, 1, None, None) == -1
+    assert lib.tdde_nccl_unique_id(None) == -1
+    lib.tdde_group_destroy(None)                      # NULL is allowed
+
+
 def test_reference_arm_prints_on_rank0_only():
     """bench.py --impl reference under a 2-rank launch: rank 0 prints the JSON line, other ranks exit 0 silently."""
     import json
