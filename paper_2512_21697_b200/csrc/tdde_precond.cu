@@ -20,8 +20,14 @@
 #include "tdde_reduce.cuh"
 
 #define PC_NT 32
+// Schur chain, W > 8: the block rows do not fit a second register set, so they are prefetched into L1 (prefetch.global.L1) four steps
+// ahead and read at use, and only b, m1, m2 (resp. z) are held per set (bandwidth 19: solve 0.895 -> 0.844 ms).  W <= 8 keeps two full
+// register sets: the same scheme measured slower there (HBM-scale W = 6: 0.504 -> 0.540 ms).
+#ifndef TDDE_SCHUR_L1PF
+#define TDDE_SCHUR_L1PF(W) ((W) > 8)
+#endif
 #ifndef TDDE_SCHUR_DEPTH
-#define TDDE_SCHUR_DEPTH(W) ((W) <= 8 ? 2 : 1)   // measured on B200: 3 and 4 sets spill and lose (HBM-scale solve 0.50 -> 0.56 / 0.60 ms)
+#define TDDE_SCHUR_DEPTH(W) (TDDE_SCHUR_L1PF(W) ? 4 : 2)   // full sets: 3 and 4 spill and lose (HBM-scale solve 0.50 -> 0.56 / 0.60 ms)
 #endif
 #define PC_ROWS 8
 #ifndef PC_STAGES
@@ -241,9 +247,10 @@ __global__ void __launch_bounds__(128) k_vec_spikes(const VecArgs v, const PrecA
 // one CTA barrier per step.  Software pipelining: the operands of the next step are loaded, untouched, into a second register
 // set before the block products of the current step (loops unrolled by two so the sets swap roles without copies). ----
 template <int W>
-struct SchurFwd { cplx b, m1, m2, lb[W], di[W]; };
+struct SchurFwd { cplx b, m1, m2, lb[TDDE_SCHUR_L1PF(W) ? 1 : W], di[TDDE_SCHUR_L1PF(W) ? 1 : W]; };
 template <int W>
-struct SchurBwd { cplx z, g[W]; };
+struct SchurBwd { cplx z, g[TDDE_SCHUR_L1PF(W) ? 1 : W]; };
+__device__ __forceinline__ void pf_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 
 template <int W>
 __global__ void __launch_bounds__(PC_NT* W, (W <= 6 ? 2 : 1)) k_precond_schur(const PrecArgs p) {
@@ -255,6 +262,7 @@ __global__ void __launch_bounds__(PC_NT* W, (W <= 6 ? 2 : 1)) k_precond_schur(co
   constexpr int WW = W * W;
   const cplx* Sk = p.Schur + (size_t)p.cls[a] * ns * 3 * WW + c * W;  // row c of every block
   auto sep_row = [&](int j) { return pc_lo(p, j) + pc_len(p, j) + c; };
+  constexpr bool L1PF = TDDE_SCHUR_L1PF(W);
   constexpr int D = TDDE_SCHUR_DEPTH(W);    // operand sets in flight: each is 2 W + 3 complex registers in the forward pass
   // ---------------- forward ----------------
   auto ffetch = [&](int j, SchurFwd<W>& o) {
@@ -262,17 +270,24 @@ __global__ void __launch_bounds__(PC_NT* W, (W <= 6 ? 2 : 1)) k_precond_schur(co
     o.b = p.x[(size_t)sep_row(j) * ld + a];
     o.m1 = p.rsp[((size_t)j * W + c) * ld + a];
     o.m2 = p.rsm[((size_t)(j + 1) * W + c) * ld + a];
+    const cplx* rb = Sk + (size_t)j * 3 * WW;                       // rows c of B_j D'^-1_{j-1} and of D'^-1_j: W x 16 bytes each
+    if (L1PF) { pf_l1(rb); pf_l1(rb + W - 1); pf_l1(rb + WW); pf_l1(rb + WW + W - 1); }
+    else {
 #pragma unroll
-    for (int q = 0; q < W; ++q) { o.lb[q] = __ldg(Sk + (size_t)j * 3 * WW + q); o.di[q] = __ldg(Sk + (size_t)j * 3 * WW + WW + q); }
+      for (int q = 0; q < (L1PF ? 1 : W); ++q) { o.lb[q] = __ldg(rb + q); o.di[q] = __ldg(rb + WW + q); }
+    }
   };
   // r'_{j-1} is in sh[(j-1) & 1]; publishes r'_j in sh[j & 1], then row c of z_j
+#define LB(q) (L1PF ? __ldg(Sk + (size_t)j * 3 * WW + (q)) : o.lb[L1PF ? 0 : (q)])
+#define DI(q) (L1PF ? __ldg(Sk + (size_t)j * 3 * WW + WW + (q)) : o.di[L1PF ? 0 : (q)])
+#define GG(q) (L1PF ? __ldg(Sk + (size_t)j * 3 * WW + 2 * WW + (q)) : o.g[L1PF ? 0 : (q)])
   auto fstep = [&](int j, const SchurFwd<W>& o) {
     cplx r0 = make_double2(o.b.x - o.m1.x - o.m2.x, o.b.y - o.m1.y - o.m2.y), r1 = make_double2(0, 0);
     if (j > 0) {
 #pragma unroll
       for (int q = 0; q < W; q += 2) {
-        cfms(r0, o.lb[q], sh[(j - 1) & 1][q][lane]);
-        if (q + 1 < W) cfms(r1, o.lb[q + 1], sh[(j - 1) & 1][q + 1][lane]);
+        cfms(r0, LB(q), sh[(j - 1) & 1][q][lane]);
+        if (q + 1 < W) cfms(r1, LB(q + 1), sh[(j - 1) & 1][q + 1][lane]);
       }
     }
     sh[j & 1][c][lane] = cadd(r0, r1);
@@ -280,8 +295,8 @@ __global__ void __launch_bounds__(PC_NT* W, (W <= 6 ? 2 : 1)) k_precond_schur(co
     cplx z0 = make_double2(0, 0), z1 = make_double2(0, 0);
 #pragma unroll
     for (int q = 0; q < W; q += 2) {
-      cfma(z0, o.di[q], sh[j & 1][q][lane]);
-      if (q + 1 < W) cfma(z1, o.di[q + 1], sh[j & 1][q + 1][lane]);
+      cfma(z0, DI(q), sh[j & 1][q][lane]);
+      if (q + 1 < W) cfma(z1, DI(q + 1), sh[j & 1][q + 1][lane]);
     }
     p.rsp[((size_t)j * W + c) * ld + a] = cadd(z0, z1);
   };
@@ -306,16 +321,19 @@ __global__ void __launch_bounds__(PC_NT* W, (W <= 6 ? 2 : 1)) k_precond_schur(co
   auto bfetch = [&](int j, SchurBwd<W>& o) {
     if (j < 0) return;
     o.z = p.rsp[((size_t)j * W + c) * ld + a];
+    if (L1PF) { pf_l1(Sk + (size_t)j * 3 * WW + 2 * WW); pf_l1(Sk + (size_t)j * 3 * WW + 2 * WW + W - 1); }
+    else {
 #pragma unroll
-    for (int q = 0; q < W; ++q) o.g[q] = __ldg(Sk + (size_t)j * 3 * WW + 2 * WW + q);
+      for (int q = 0; q < (L1PF ? 1 : W); ++q) o.g[q] = __ldg(Sk + (size_t)j * 3 * WW + 2 * WW + q);
+    }
   };
   auto bstep = [&](int j, const SchurBwd<W>& o) {
     cplx x0 = o.z, x1 = make_double2(0, 0);
     if (j + 1 < ns) {
 #pragma unroll
       for (int q = 0; q < W; q += 2) {
-        cfms(x0, o.g[q], sh[(j + 1) & 1][q][lane]);
-        if (q + 1 < W) cfms(x1, o.g[q + 1], sh[(j + 1) & 1][q + 1][lane]);
+        cfms(x0, GG(q), sh[(j + 1) & 1][q][lane]);
+        if (q + 1 < W) cfms(x1, GG(q + 1), sh[(j + 1) & 1][q + 1][lane]);
       }
     }
     const cplx xv = cadd(x0, x1);
@@ -338,6 +356,10 @@ __global__ void __launch_bounds__(PC_NT* W, (W <= 6 ? 2 : 1)) k_precond_schur(co
     }
   }
 }
+
+#undef LB
+#undef DI
+#undef GG
 
 // ---- P2b: with every x_S known, A_IS x_S for the interiors next to each separator: the last w rows of interior j (into r(+)_j)
 // and the first w rows of interior j+1 (into r(-)_{j+1}).  One thread per (separator, channel). ----
