@@ -438,11 +438,11 @@ static int create_impl(tdde_handle* h, const tdde_c64* S_band, const tdde_c64* H
         }
         h->seg_len_m = best_seg;
         if (const char* env = std::getenv("TDDE_MMA_SEG")) h->seg_len_m = std::max(8, std::atoi(env) / 8 * 8);
-        // Start of step as block pass + DMMA coupling apply.  Measured on B200 (ms per step, split / one H-apply + S-apply): HBM-scale
-        // T = 7, W = 6: 7.85 / 8.01; W = 9: 10.74 / 10.60 (the two 19-entry windows of the block pass do not fit); Large T = 5:
-        // 1.566 / 1.554.  So: only where the register-window kernel needs its two-group term split (T >= 6) and the block pass keeps
-        // both windows in registers (W <= 6).  TDDE_SPLIT_START / TDDE_NO_SPLIT_START force it (tests).
-        h->split_start = h->use_subst && ((T >= 6 && h->bW <= 6) || std::getenv("TDDE_SPLIT_START"));
+        // Start of step as block pass + DMMA coupling apply.  Measured on B200 (ms per step, split / one H-apply + S-apply), with the
+        // final block pass (at most four classes staged, tensor-map x rows): HBM-scale T = 7, W = 6: 7.85 / 8.01; W = 9: 10.19 / 10.53;
+        // Large T = 5: 1.582 / 1.550; Medium T = 5: 0.406 / 0.372.  So: where the register-window kernel needs its two-group term
+        // split (T >= 6).  TDDE_SPLIT_START / TDDE_NO_SPLIT_START force it (tests).
+        h->split_start = h->use_subst && (T >= 6 || std::getenv("TDDE_SPLIT_START"));
         if (std::getenv("TDDE_NO_SPLIT_START")) h->split_start = false;
       }
     }
