@@ -166,6 +166,29 @@ int  tdde_group_create(tdde_group** out, int32_t n_local, tdde_handle* const* ha
 int  tdde_group_propagate(tdde_group* g, tdde_c64* const* c_dev, int64_t n_steps, const double* g_table, tdde_stats* st);
 void tdde_group_destroy(tdde_group* g);                         /* the handles stay alive and become ordinary handles again */
 
+/* ---- An entry point that allocates nothing (for callers that cannot call cudaMalloc: code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it).  *out_dev = Re(c^H S c), the total probability of tdde_norm (S: PAPER.md:178-182), computed straight
+ * from device copies of the inputs -- no handle, no cudaMalloc / cudaFree / allocating library call.  It is the S-only apply with its
+ * fused norm reduction; the per-block partial sums and the completion ticket of that reduction, which the handle path keeps in
+ * buffers allocated by tdde_create, live in a file-scope `static __device__` array of TDDE_NOALLOC_MAX_BLOCKS doubles (+ ticket;
+ * 64 KB + 256 B that every GPU which loads the library holds until exit).  One block reduces TDDE_NOALLOC_ELEMS_PER_BLOCK elements, so
+ *     n_ang * n_rad <= TDDE_NOALLOC_MAX_N = 16 777 216 elements       (BASELINE "large", 6e6, fits; the HBM-scale config does not);
+ * larger problems are rejected with TDDE_EINVAL and a text in tdde_last_cuda_error() that names the limit.
+ *   S_band_dev : device [n_cls][n_rad][2*w0+1], the row-band layout of tdde_create;  cls_dev : device int32 [n_ang], values in [0, n_cls)
+ *   c_dev      : device, n complex128, boundary layout;  out_dev : device double[1];  cuda_stream : cudaStream_t (as void*)
+ * w0 <= 32.  Does not synchronise; *out_dev is valid when the stream reaches the end of the call's work.
+ * EVERY call on a device shares the one scratch array, which keeps the last call's contents: the call clears the ticket itself (a
+ * memset node, no allocation) and overwrites every partial it reads, but two calls that overlap on the GPU (different streams, or two
+ * graphs replayed concurrently) race on it -- serialise them.  tdde_snorm_noalloc_setup() resolves the array's device address
+ * (cudaGetSymbolAddress, once per device, on the current device); the entry point does the same on its first call on a device, so call
+ * the set-up once before capturing a graph.  Errors: TDDE_EINVAL, TDDE_ECUDA. */
+#define TDDE_NOALLOC_ELEMS_PER_BLOCK 2048
+#define TDDE_NOALLOC_MAX_BLOCKS 8192
+#define TDDE_NOALLOC_MAX_N ((int64_t)TDDE_NOALLOC_ELEMS_PER_BLOCK * TDDE_NOALLOC_MAX_BLOCKS)
+int tdde_snorm_noalloc_setup(void);
+int tdde_snorm_noalloc(int32_t n_ang, int32_t n_rad, int32_t n_cls, int32_t w0, const tdde_c64* S_band_dev, const int32_t* cls_dev,
+                       const tdde_c64* c_dev, double* out_dev, void* cuda_stream);
+
 /* Which operator-apply kernel the handle uses: 1 = banded A_L held in registers, 2 = general sparse A_L staged in shared memory
  * (x tile by TMA), 0 = unstaged generic CSR fall-back. */
 int tdde_apply_path(const tdde_handle* h);

@@ -19,7 +19,7 @@ LIB_PATH = os.environ.get("TDDE_LIB_PATH", os.path.join(_HERE, "libtdde.so"))
 EXPORTS = [
     "tdde_create", "tdde_step", "tdde_propagate", "tdde_norm", "tdde_apply", "tdde_precond",
     "tdde_propagate_host", "tdde_step_forced", "tdde_apply_coupling", "tdde_time_kernel", "tdde_fp64_peak", "tdde_fp64_pipe_probe", "tdde_launch_count",
-    "tdde_apply_path", "tdde_iter_apply_kernel", "tdde_nccl_unique_id", "tdde_group_create", "tdde_group_propagate", "tdde_group_destroy", "tdde_set_eigenstates", "tdde_project", "tdde_eigensolve", "tdde_selftest_partition", "tdde_selftest_mma_frags", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
+    "tdde_apply_path", "tdde_snorm_noalloc_setup", "tdde_snorm_noalloc", "tdde_iter_apply_kernel", "tdde_nccl_unique_id", "tdde_group_create", "tdde_group_propagate", "tdde_group_destroy", "tdde_set_eigenstates", "tdde_project", "tdde_eigensolve", "tdde_selftest_partition", "tdde_selftest_mma_frags", "tdde_paper_variant", "tdde_destroy", "tdde_strerror", "tdde_last_cuda_error", "tdde_version",
 ]
 
 STATUS = {0: "TDDE_OK", -1: "TDDE_EINVAL", -2: "TDDE_ENOMEM", -3: "TDDE_ECUDA", -4: "TDDE_ESINGULAR",
@@ -113,6 +113,10 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.tdde_group_propagate.restype = C.c_int
     lib.tdde_group_destroy.argtypes = [vp]
     lib.tdde_group_destroy.restype = None
+    lib.tdde_snorm_noalloc_setup.argtypes = []
+    lib.tdde_snorm_noalloc_setup.restype = C.c_int
+    lib.tdde_snorm_noalloc.argtypes = [i32, i32, i32, i32, vp, vp, vp, vp, vp]
+    lib.tdde_snorm_noalloc.restype = C.c_int
     lib.tdde_destroy.argtypes = [vp]
     lib.tdde_destroy.restype = None
     lib.tdde_strerror.argtypes = [C.c_int]
@@ -398,3 +402,24 @@ class TddeGroup:
             self.close()
         except Exception:
             pass
+
+
+NOALLOC_MAX_N = 2048 * 8192      # TDDE_NOALLOC_MAX_N of include/tdde.h
+
+
+def snorm_noalloc_setup():
+    """Resolve the static scratch array's device address on the current device (tdde_snorm_noalloc_setup)."""
+    lib = load_library()
+    _check(lib, lib.tdde_snorm_noalloc_setup(), "tdde_snorm_noalloc_setup")
+
+
+def snorm_noalloc(n_ang: int, n_rad: int, n_cls: int, w0: int, S_dev, cls_dev, c_dev, out_dev, stream=None, check: bool = True) -> int:
+    """*out_dev = Re(c^H S c) without any allocation (tdde_snorm_noalloc).  S_dev: CUDA complex128 [n_cls, n_rad, 2 w0 + 1] (row band),
+    cls_dev: CUDA int32 [n_ang], c_dev: CUDA complex128 [n_ang * n_rad], out_dev: CUDA float64 [1].  Argument marshalling only."""
+    lib = load_library()
+    st = C.c_void_p(stream.cuda_stream) if stream is not None else None
+    rc = lib.tdde_snorm_noalloc(n_ang, n_rad, n_cls, w0, C.c_void_p(S_dev.data_ptr()), C.c_void_p(cls_dev.data_ptr()),
+                                C.c_void_p(c_dev.data_ptr()), C.c_void_p(out_dev.data_ptr()), st)
+    if check:
+        _check(lib, rc, "tdde_snorm_noalloc")
+    return rc

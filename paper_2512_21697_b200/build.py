@@ -19,7 +19,7 @@ ROOT = os.path.dirname(HERE)
 INCLUDE = os.path.join(ROOT, "include")
 OUT = os.environ.get("TDDE_LIB_OUT", os.path.join(HERE, "libtdde.so"))      # overrides: build-variant experiments
 EXTRA = os.environ.get("TDDE_NVCC_FLAGS", "").split()
-SOURCES = ["tdde_apply.cu", "tdde_apply_mma.cu", "tdde_apply_block2.cu", "tdde_apply_sparse.cu", "tdde_vec.cu", "tdde_precond.cu", "tdde_partition.cu", "tdde_create.cu", "tdde_driver.cu", "tdde_shard.cu", "tdde_misc.cu", "tdde_eigen.cu", "tdde_paper_variant.cu"]
+SOURCES = ["tdde_apply.cu", "tdde_apply_mma.cu", "tdde_apply_block2.cu", "tdde_apply_sparse.cu", "tdde_vec.cu", "tdde_precond.cu", "tdde_partition.cu", "tdde_create.cu", "tdde_driver.cu", "tdde_shard.cu", "tdde_misc.cu", "tdde_noalloc.cu", "tdde_eigen.cu", "tdde_paper_variant.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-DTDDE_WITH_BENCH"]
 
