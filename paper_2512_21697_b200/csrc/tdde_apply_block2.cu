@@ -7,13 +7,21 @@
 #include "tdde_reduce.cuh"
 
 #define B2_NC TDDE_AP_NC
+#ifndef B2_JC
 #define B2_JC 4
+#endif
 #ifndef B2_NST
 #define B2_NST 3      // measured: 4 stages lose (HBM-scale step 7.87 -> 8.36 ms)
 #endif
 #define B2_MAXC TDDE_AP_MAXC
+#ifndef B2_RU
+#define B2_RU 1
+#endif
+#ifndef B2_MINB9
+#define B2_MINB9 1
+#endif
 #ifndef B2_MINB6
-#define B2_MINB6 3
+#define B2_MINB6 2
 #endif
 
 namespace {
@@ -51,16 +59,19 @@ struct Block2Plan {
 
 // p.x -> p.y = oscale * (blk) x, p.y2 = (blk2) x; blk / blk2 in column-band form [n_cls][n_rad][2W+1]
 template <int W>
-__global__ void __launch_bounds__(B2_NC, (W <= 3 ? 4 : W <= 6 ? B2_MINB6 : 2)) k_block_dual(const __grid_constant__ ApplyArgs p, const cplx* __restrict__ blk2) {
+__global__ void __launch_bounds__(2 * B2_NC, (W <= 3 ? 4 : W <= 6 ? B2_MINB6 : B2_MINB9)) k_block_dual(const __grid_constant__ ApplyArgs p, const cplx* __restrict__ blk2) {
   using PL = Block2Plan<W>;
-  constexpr int ND = PL::ND, JC = B2_JC;
+  constexpr int ND = PL::ND, JC = B2_JC, RU = B2_RU;
   if (p.guard == 2 && (p.red.st->stalled | (p.red.st->status != 0))) return;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   cplx* stage_base = reinterpret_cast<cplx*>(smem_raw);
   const int CS = PL::cs(p.n_cta_cls), STAGE = PL::stage(p.n_cta_cls);
   uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)B2_NST * STAGE * sizeof(cplx));
 
-  const int tid = threadIdx.x, ld = p.ld, n_rad = p.n_rad;
+  // 256 threads: threads [0, 128) form (blk) x, threads [128, 256) form (blk2) x from the same staged x rows -- one 2W+1 window per
+  // thread instead of two (half the registers, twice the warps per SM)
+  const int tid = threadIdx.x % B2_NC, op = threadIdx.x / B2_NC, ld = p.ld, n_rad = p.n_rad;
+  const cplx* const blk_g = op ? blk2 : p.blk;
   const int a0 = blockIdx.x * B2_NC, a = a0 + tid;
   const bool lane_ok = a >= p.own_lo && a < p.own_hi;          // own_hi <= ld
   const int ac = a < ld ? a : ld - 1;
@@ -72,8 +83,8 @@ __global__ void __launch_bounds__(B2_NC, (W <= 3 ? 4 : W <= 6 ? B2_MINB6 : 2)) k
   const int* cta_cls = p.cta_cls + blockIdx.x * B2_MAXC;
   const int nch = min(B2_NC, ld - a0);                        // channels of this CTA inside the vector
   if (nch < B2_NC)
-    for (int q = tid; q < B2_NST * STAGE; q += B2_NC) stage_base[q] = make_double2(0, 0);
-  if (tid == 0) {
+    for (int q = threadIdx.x; q < B2_NST * STAGE; q += 2 * B2_NC) stage_base[q] = make_double2(0, 0);
+  if (threadIdx.x == 0) {
     for (int q = 0; q < B2_NST; ++q) b2_bar_init(&full[q], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -109,46 +120,44 @@ __global__ void __launch_bounds__(B2_NC, (W <= 3 ? 4 : W <= 6 ? B2_MINB6 : 2)) k
         b2_bulk(st + 2 * CS + (size_t)r * B2_NC, p.x + (size_t)(j + r) * ld + a0, (uint32_t)nch * sizeof(cplx), bar);
     }
   };
-  if (tid == 0)
+  if (threadIdx.x == 0)
     for (int c = 0; c < B2_NST && c < nchunks; ++c) issue(c);
 
-  cplx w1[ND], w2[ND];
+  cplx w1[ND];
 #pragma unroll
-  for (int e = 0; e < ND; ++e) { w1[e] = make_double2(0, 0); w2[e] = make_double2(0, 0); }
+  for (int e = 0; e < ND; ++e) w1[e] = make_double2(0, 0);
   for (int c = 0; c < nchunks; ++c) {
     const cplx* st = stage_base + (size_t)(c % B2_NST) * STAGE;
     const int jc0 = jlo + c * JC;
     const int nr_real = min(JC, jhi - jc0), nr_all = min(JC, jend - jc0);
     if (nr_real > 0) b2_wait(&full[c % B2_NST], (c / B2_NST) & 1);
-#pragma unroll(W >= 6 ? 1 : 2)
+#pragma unroll(RU)
     for (int r = 0; r < JC; ++r) {
       if (r < nr_all) {
         if (r < nr_real) {
           const cplx x0 = st[2 * CS + r * B2_NC + tid];
           if (slot >= 0) {
-            const cplx* c1 = st + ((size_t)slot * JC + r) * ND;
-            const cplx* c2 = c1 + CS;
+            const cplx* c1 = st + (size_t)op * CS + ((size_t)slot * JC + r) * ND;
 #pragma unroll
-            for (int e = 0; e < ND; ++e) { cfma(w1[e], c1[e], x0); cfma(w2[e], c2[e], x0); }
+            for (int e = 0; e < ND; ++e) cfma(w1[e], c1[e], x0);
           } else {
-            const cplx* c1 = p.blk + cls_off + (size_t)(jc0 + r) * ND;
-            const cplx* c2 = blk2 + cls_off + (size_t)(jc0 + r) * ND;
+            const cplx* c1 = blk_g + cls_off + (size_t)(jc0 + r) * ND;
 #pragma unroll
-            for (int e = 0; e < ND; ++e) { cfma(w1[e], __ldg(c1 + e), x0); cfma(w2[e], __ldg(c2 + e), x0); }
+            for (int e = 0; e < ND; ++e) cfma(w1[e], __ldg(c1 + e), x0);
           }
         }
         const int i = jc0 + r - W;
         if (i >= i0 && lane_ok) {
-          p.y[(size_t)i * ld + a] = cmul(p.oscale, w1[0]);
-          p.y2[(size_t)i * ld + a] = w2[0];
+          if (op == 0) p.y[(size_t)i * ld + a] = cmul(p.oscale, w1[0]);
+          else p.y2[(size_t)i * ld + a] = w1[0];
         }
 #pragma unroll
-        for (int e = 0; e < ND - 1; ++e) { w1[e] = w1[e + 1]; w2[e] = w2[e + 1]; }
-        w1[ND - 1] = make_double2(0, 0); w2[ND - 1] = make_double2(0, 0);
+        for (int e = 0; e < ND - 1; ++e) w1[e] = w1[e + 1];
+        w1[ND - 1] = make_double2(0, 0);
       }
     }
     __syncthreads();                                            // everybody is done with stage c % NST
-    if (tid == 0 && c + B2_NST < nchunks) issue(c + B2_NST);
+    if (threadIdx.x == 0 && c + B2_NST < nchunks) issue(c + B2_NST);
   }
 }
 
@@ -163,7 +172,7 @@ static int launch_block_dual_w(const ApplyArgs& a, const cplx* blk2, cudaStream_
     if (dev >= 0 && dev < 64) attr_set[dev] = true;
   }
   dim3 grid((a.ld + B2_NC - 1) / B2_NC, (a.n_rad + a.seg_len - 1) / a.seg_len);
-  k_block_dual<W><<<grid, B2_NC, smem, s>>>(a, blk2);
+  k_block_dual<W><<<grid, 2 * B2_NC, smem, s>>>(a, blk2);
   return 1;
 }
 
